@@ -1,0 +1,146 @@
+/* nk.h -- C-ABI of libnk: matrix-free, sum-factorised spectral/hp elemental
+ * operators on batches ("blocks") of like elements, fp64, one NVIDIA B200.
+ *
+ * Citations: P:<n> = line n of the paper text (arxiv/paper_2606_20917,
+ * "NektarIR"); A<n> = reading n in DESIGN.md section 3.
+ *
+ * A *block* is a set of elements with one shape, one polynomial
+ * order P, one quadrature order Q and one "deformed" flag.  Here a block is the
+ * triple (nk_basis, nk_geom, nelem) plus caller-owned field pointers.
+ *
+ * Conventions
+ *   - nm = P+1 modes per direction (A1); Q quadrature points per direction;
+ *     Nq = Q^3 points per element, point index n = i + Q*(j + Q*k), direction-1
+ *     index fastest (A11); Nm modes per element in the nest order of Eq. 17
+ *     (A3): p outermost, r innermost.
+ *   - fields are fp64, element-major: coefficients [nelem][Nm], point values
+ *     [nelem][Nq].  All field pointers are DEVICE pointers owned by the caller
+ *     unless the name of the call says "_host".  in/out must not alias.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = default stream).  Calls
+ *     enqueue work and return without synchronising (except *_host calls and
+ *     nk_geom_upload with host input, which synchronise `stream`).
+ *   - handles (nk_basis, nk_geom) are created and destroyed by the library;
+ *     every other buffer stays the caller's.
+ *   - errors are return codes; nk_last_error() gives a thread-local message.
+ *     Nothing throws across the boundary.  There is no CPU fallback: without a
+ *     CUDA device every compute call returns NK_ERR_CUDA.
+ */
+#ifndef NK_H
+#define NK_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    NK_OK = 0,
+    NK_ERR_INVALID_ARG = 1,
+    NK_ERR_UNSUPPORTED = 2,    /* (shape,P,Q) outside the instantiation table */
+    NK_ERR_SHAPE_MISMATCH = 3, /* basis / geom / nelem do not belong together */
+    NK_ERR_ALLOC = 4,
+    NK_ERR_CUDA = 5
+} nk_status;
+
+typedef enum { NK_HEX = 0, NK_TET = 1, NK_PRISM = 2 } nk_shape;
+
+/* tables readable through nk_basis_get_table (for tests) */
+typedef enum {
+    NK_TAB_NODES = 0,   /* z^(dir)[Q]                                              */
+    NK_TAB_WEIGHTS = 1, /* w^(dir)[Q], collapse Jacobian folded in (A16)           */
+    NK_TAB_DERIV = 2,   /* D^(dir)[Q][Q], D[i][r] = h_r'(z_i) (Eq. 22; A5)  */
+    NK_TAB_PSI = 3      /* dir 0: psi^a_p(z1_i) as [Q][nm];
+                           dir 1: hex/prism psi^a_q(z2_j) as [Q][nm];
+                                  tet psi^b_{pq}(z2_j) as [Q][nm(nm+1)/2], column (p,q) = sum_{a<p}(nm-a)+q;
+                           dir 2: hex psi^a_r(z3_k) as [Q][nm];
+                                  tet/prism psi^b_{sr}(z3_k) as [Q][nm(nm+1)/2], column (s,r) (A7)  */
+} nk_table;
+
+typedef struct nk_basis nk_basis; /* opaque: shape, P, Q, host tables (+ device copies, made lazily) */
+typedef struct nk_geom nk_geom;   /* opaque: nelem, deformed flag, repacked device streams          */
+
+/* ---- basis / quadrature precompute (host only; needs no GPU) ----------------------------------
+ * Modified C0 basis (A7, A8) with Gauss-Lobatto-Legendre points on hexes, GLL x Gauss-Radau-Jacobi(1,0)
+ * x GRJ(2,0) on tets, GLL x GLL x GRJ(1,0) on prisms (A9).  Supported: Q == P+2 with
+ * hex P in 1..10, tet and prism P in 1..8; anything else returns NK_ERR_UNSUPPORTED.               */
+nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** out);
+nk_status nk_basis_destroy(nk_basis* b);
+int nk_basis_num_modes(const nk_basis* b);  /* Nm; -1 if b is NULL */
+int nk_basis_num_points(const nk_basis* b); /* Nq = Q^3           */
+int nk_basis_interleave(const nk_basis* b); /* E: elements per thread block = width of the internal
+                                               element-interleaved layout (A12) */
+/* copies table `which` of direction dir (0,1,2) into host_out; cap = capacity in doubles.
+ * NK_ERR_INVALID_ARG if cap is too small.  *count (may be NULL) receives the number of doubles.    */
+nk_status nk_basis_get_table(const nk_basis* b, int which, int dir, double* host_out, size_t cap, size_t* count);
+/* standard-element coordinates xi of the Nq quadrature points, xi_out[n][3] (cap in doubles >= 3*Nq):
+ * the collapsed nodes eta mapped by the inverse of Eq. 13 (A2).  For building geometry inputs. */
+nk_status nk_basis_get_points(const nk_basis* b, double* xi_out, size_t cap);
+/* storage rank of mode (p,q,r) (Eq. 18; A3); -1 if (p,q,r) is not a mode of the expansion   */
+int nk_basis_mode_index(const nk_basis* b, int p, int q, int r);
+
+/* ---- geometry (A13, A14) -------------------------------------------------
+ * dxi_dx: [nelem][npt][3][3], entry [j][i] = d xi_j / d x_i, xi = STANDARD-element coordinates (the
+ *         collapsed eta of Eq. 13 are internal); detJ: [nelem][npt] > 0.
+ * npt = 1 if !deformed (affine: constant factors per element), Nq if deformed (point index n as above).
+ * on_device: 0 = the two pointers are host memory, 1 = device memory.  The caller keeps its arrays;
+ * the library builds its own element-interleaved streams:
+ *   metric stream  G = w|J| (dxi/dx)(dxi/dx)^T (6, symmetric) + w|J| (1)   -- Laplacian / Helmholtz / mass / iprod
+ *   factor stream  dxi/dx (9) + w|J| (1)                                    -- physderiv / iprod_deriv
+ * with the collapsed-coordinate chain of Eq. 23 (A17) and the quadrature weights folded in when
+ * deformed.  nelem == 0 is valid (every apply is then a no-op).                                      */
+nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
+                         const double* detJ, int on_device, void* stream, nk_geom** out);
+nk_status nk_geom_destroy(nk_geom* g);
+int64_t nk_geom_num_elements(const nk_geom* g);
+
+/* ---- elemental operators --------------------------------------------------------------------- */
+/* BwdTrans, u = B uhat (Eq. 14-17): coeffs [nelem][Nm] -> phys [nelem][Nq].             */
+nk_status nk_bwdtrans(const nk_basis* b, int64_t nelem, const double* coeffs, double* phys, void* stream);
+/* IProductWRTBase, uhat = B^T W u (Eq. 19-21): phys [nelem][Nq] -> coeffs [nelem][Nm].  */
+nk_status nk_iprod(const nk_basis* b, const nk_geom* g, const double* phys, double* coeffs, void* stream);
+/* PhysDeriv (Eq. 22, 23, 9): phys -> d_i = du/dx_i, each [nelem][Nq].
+ * A NULL d_i skips that component.                                                                 */
+nk_status nk_physderiv(const nk_basis* b, const nk_geom* g, const double* phys, double* d0, double* d1,
+                       double* d2, void* stream);
+/* IProductWRTDerivBase (Eq. 7): coeffs_m = sum_n W_n sum_i (d phi_m/d x_i)(xi_n) g_i[n].
+ * A NULL g_i counts as zero.                                                                       */
+nk_status nk_iprod_deriv(const nk_basis* b, const nk_geom* g, const double* g0, const double* g1,
+                         const double* g2, double* coeffs, void* stream);
+/* M uhat = B^T W B uhat (Eq. 7).                                                      */
+nk_status nk_mass_apply(const nk_basis* b, const nk_geom* g, const double* in, double* out, void* stream);
+/* L uhat = sum_i (D_xi B)^T W (D_xi B) uhat (Eq. 7).                                         */
+nk_status nk_laplacian_apply(const nk_basis* b, const nk_geom* g, const double* in, double* out, void* stream);
+/* out = (L + lambda M) in (Eq. 5-6; A6), one fused kernel: point data never leaves the SM. */
+nk_status nk_helmholtz_apply(const nk_basis* b, const nk_geom* g, double lambda, const double* in,
+                             double* out, void* stream);
+
+/* several blocks (possibly of different shape / order) in one call, e.g. a hybrid prism + tet mesh   */
+typedef struct {
+    const nk_basis* basis;
+    const nk_geom* geom;
+    const double* in; /* device [nelem][Nm] */
+    double* out;      /* device [nelem][Nm] */
+} nk_block;
+nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double lambda, void* stream);
+
+/* End-to-end variant with HOST field buffers: copies host_in to an internal device buffer, applies the
+ * Helmholtz operator and copies the result back into host_out; synchronises `stream` before returning.
+ * Pinned host memory makes the copies asynchronous DMA; pageable memory works but is slower.         */
+nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g, double lambda, const double* host_in,
+                                  double* host_out, void* stream);
+
+/* ---- diagnostics ----------------------------------------------------------------------------- */
+/* Register-only DFMA chains on every SM for about `iters` x 4096 FMAs per thread; *tflops receives the
+ * sustained fp64 rate (2 flop per FMA).  This is the measured FP64 roofline denominator.            */
+nk_status nk_probe_fp64_peak(int iters, double* tflops, double* ms);
+/* number of kernels this library has launched from the calling process so far                      */
+int64_t nk_launch_count(void);
+const char* nk_last_error(void);
+const char* nk_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NK_H */

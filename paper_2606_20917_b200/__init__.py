@@ -1,0 +1,20 @@
+"""paper_2606_20917_b200 -- Python face of libnk (include/nk.h): B200-native, matrix-free,
+sum-factorised spectral/hp elemental operators (arxiv/paper_2606_20917 hot path).
+
+The binding (binding.py) only marshals arguments; every step of the path runs in the CUDA
+kernels of libnk.so.  Names are resolved lazily so that `python -m paper_2606_20917_b200.build`
+can run before the library exists; any other use without a built libnk.so raises.
+"""
+_EXPORTS = ("lib", "NkError", "Basis", "Geom", "HEX", "TET", "PRISM", "bwdtrans", "iprod", "physderiv",
+            "iprod_deriv", "mass_apply", "laplacian_apply", "helmholtz_apply", "helmholtz_apply_blocks",
+            "helmholtz_apply_host", "probe_fp64_peak", "launch_count", "version", "LIB_PATH", "DECLARED_SYMBOLS")
+
+
+def __getattr__(name):
+    if name in _EXPORTS:
+        from . import binding
+        return getattr(binding, name)
+    raise AttributeError(name)
+
+
+__all__ = list(_EXPORTS)

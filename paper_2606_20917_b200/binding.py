@@ -1,0 +1,213 @@
+"""ctypes binding of libnk.so -- same names as include/nk.h, argument marshalling only.
+
+PyTorch is used for device memory and streams; tensors are passed as raw pointers.  There is no
+Python or CPU implementation behind these calls: if libnk.so is missing the import fails.
+"""
+import ctypes as C
+import os
+
+import torch
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libnk.so")
+HEX, TET, PRISM = 0, 1, 2
+TAB_NODES, TAB_WEIGHTS, TAB_DERIV, TAB_PSI = 0, 1, 2, 3
+
+if not os.path.exists(LIB_PATH):
+    raise ImportError("libnk.so not built (%s): run `python -m paper_2606_20917_b200.build`; "
+                      "there is no CPU fallback" % LIB_PATH)
+lib = C.CDLL(LIB_PATH)
+
+_p, _d, _i, _i64, _sz = C.c_void_p, C.c_double, C.c_int, C.c_int64, C.c_size_t
+_SIG = {
+    "nk_basis_create": (_i, [_i, _i, _i, C.POINTER(_p)]),
+    "nk_basis_destroy": (_i, [_p]),
+    "nk_basis_num_modes": (_i, [_p]),
+    "nk_basis_num_points": (_i, [_p]),
+    "nk_basis_interleave": (_i, [_p]),
+    "nk_basis_get_table": (_i, [_p, _i, _i, C.POINTER(_d), _sz, C.POINTER(_sz)]),
+    "nk_basis_mode_index": (_i, [_p, _i, _i, _i]),
+    "nk_basis_get_points": (_i, [_p, C.POINTER(_d), _sz]),
+    "nk_geom_upload": (_i, [_p, _i64, _i, _p, _p, _i, _p, C.POINTER(_p)]),
+    "nk_geom_destroy": (_i, [_p]),
+    "nk_geom_num_elements": (_i64, [_p]),
+    "nk_bwdtrans": (_i, [_p, _i64, _p, _p, _p]),
+    "nk_iprod": (_i, [_p, _p, _p, _p, _p]),
+    "nk_physderiv": (_i, [_p, _p, _p, _p, _p, _p, _p]),
+    "nk_iprod_deriv": (_i, [_p, _p, _p, _p, _p, _p, _p]),
+    "nk_mass_apply": (_i, [_p, _p, _p, _p, _p]),
+    "nk_laplacian_apply": (_i, [_p, _p, _p, _p, _p]),
+    "nk_helmholtz_apply": (_i, [_p, _p, _d, _p, _p, _p]),
+    "nk_helmholtz_apply_blocks": (_i, [_i, _p, _d, _p]),
+    "nk_helmholtz_apply_host": (_i, [_p, _p, _d, _p, _p, _p]),
+    "nk_probe_fp64_peak": (_i, [_i, C.POINTER(_d), C.POINTER(_d)]),
+    "nk_launch_count": (_i64, []),
+    "nk_last_error": (C.c_char_p, []),
+    "nk_version": (C.c_char_p, []),
+}
+DECLARED_SYMBOLS = tuple(_SIG)
+for _name, (_res, _args) in _SIG.items():
+    _f = getattr(lib, _name)          # AttributeError here = the .so does not export what nk.h declares
+    _f.restype, _f.argtypes = _res, _args
+
+
+class NkBlock(C.Structure):
+    _fields_ = [("basis", _p), ("geom", _p), ("inp", _p), ("out", _p)]
+
+
+class NkError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("nk_status %d: %s" % (code, msg))
+        self.code = code
+
+
+def _check(code):
+    if code != 0:
+        raise NkError(code, lib.nk_last_error().decode())
+
+
+def _ptr(t, allow_none=False):
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError("tensor required")
+    if t.dtype != torch.float64 or not t.is_contiguous():
+        raise ValueError("libnk takes contiguous float64 tensors")
+    return t.data_ptr()
+
+
+def _dev_ptr(t, allow_none=False):
+    if t is not None and not t.is_cuda:
+        raise ValueError("device tensor required (libnk has no CPU path)")
+    return _ptr(t, allow_none)
+
+
+def _stream(stream=None):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return stream.cuda_stream
+
+
+class Basis:
+    """nk_basis handle (host precompute only; needs no GPU)."""
+
+    def __init__(self, shape, P, Q=None):
+        Q = P + 2 if Q is None else Q
+        h = _p()
+        _check(lib.nk_basis_create(shape, P, Q, C.byref(h)))
+        self.h, self.shape, self.P, self.Q = h, shape, P, Q
+        self.num_modes = lib.nk_basis_num_modes(h)
+        self.num_points = lib.nk_basis_num_points(h)
+        self.interleave = lib.nk_basis_interleave(h)
+
+    def table(self, which, direction):
+        n = _sz()
+        _check(lib.nk_basis_get_table(self.h, which, direction, None, 0, C.byref(n)))
+        buf = (_d * n.value)()
+        _check(lib.nk_basis_get_table(self.h, which, direction, buf, n.value, None))
+        return torch.tensor(list(buf), dtype=torch.float64)
+
+    def points(self):
+        """xi [Nq][3] of the quadrature points (input to geometry generators)."""
+        buf = (_d * (3 * self.num_points))()
+        _check(lib.nk_basis_get_points(self.h, buf, 3 * self.num_points))
+        return torch.tensor(list(buf), dtype=torch.float64).reshape(self.num_points, 3)
+
+    def mode_index(self, p, q, r):
+        return lib.nk_basis_mode_index(self.h, p, q, r)
+
+    def close(self):
+        if self.h:
+            lib.nk_basis_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+class Geom:
+    """nk_geom handle.  dxi_dx [nelem][npt][3][3], detJ [nelem][npt]; host or device tensors."""
+
+    def __init__(self, basis, dxi_dx, detJ, deformed, stream=None):
+        nelem = detJ.shape[0]
+        npt = basis.num_points if deformed else 1
+        if tuple(dxi_dx.shape) != (nelem, npt, 3, 3) or tuple(detJ.shape) != (nelem, npt):
+            raise ValueError("geometry shapes must be [nelem][%d][3][3] and [nelem][%d]" % (npt, npt))
+        if dxi_dx.is_cuda != detJ.is_cuda:
+            raise ValueError("dxi_dx and detJ must live on the same side")
+        h = _p()
+        _check(lib.nk_geom_upload(basis.h, nelem, int(bool(deformed)), _ptr(dxi_dx), _ptr(detJ),
+                                  int(dxi_dx.is_cuda), _stream(stream), C.byref(h)))
+        self.h, self.basis, self.nelem, self.deformed = h, basis, nelem, bool(deformed)
+
+    def close(self):
+        if self.h:
+            lib.nk_geom_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def bwdtrans(basis, coeffs, phys, stream=None):
+    _check(lib.nk_bwdtrans(basis.h, coeffs.shape[0], _dev_ptr(coeffs), _dev_ptr(phys), _stream(stream)))
+
+
+def iprod(basis, geom, phys, coeffs, stream=None):
+    _check(lib.nk_iprod(basis.h, geom.h, _dev_ptr(phys), _dev_ptr(coeffs), _stream(stream)))
+
+
+def physderiv(basis, geom, phys, d0, d1, d2, stream=None):
+    _check(lib.nk_physderiv(basis.h, geom.h, _dev_ptr(phys), _dev_ptr(d0, True), _dev_ptr(d1, True),
+                            _dev_ptr(d2, True), _stream(stream)))
+
+
+def iprod_deriv(basis, geom, g0, g1, g2, coeffs, stream=None):
+    _check(lib.nk_iprod_deriv(basis.h, geom.h, _dev_ptr(g0, True), _dev_ptr(g1, True), _dev_ptr(g2, True),
+                              _dev_ptr(coeffs), _stream(stream)))
+
+
+def mass_apply(basis, geom, inp, out, stream=None):
+    _check(lib.nk_mass_apply(basis.h, geom.h, _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+
+
+def laplacian_apply(basis, geom, inp, out, stream=None):
+    _check(lib.nk_laplacian_apply(basis.h, geom.h, _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+
+
+def helmholtz_apply(basis, geom, lam, inp, out, stream=None):
+    _check(lib.nk_helmholtz_apply(basis.h, geom.h, float(lam), _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+
+
+def helmholtz_apply_blocks(blocks, lam, stream=None):
+    """blocks: sequence of (basis, geom, inp, out)."""
+    arr = (NkBlock * len(blocks))()
+    for k, (b, g, x, y) in enumerate(blocks):
+        arr[k] = NkBlock(b.h, g.h, _dev_ptr(x), _dev_ptr(y))
+    _check(lib.nk_helmholtz_apply_blocks(len(blocks), arr, float(lam), _stream(stream)))
+
+
+def helmholtz_apply_host(basis, geom, lam, host_in, host_out, stream=None):
+    if host_in.is_cuda or host_out.is_cuda:
+        raise ValueError("host tensors required")
+    _check(lib.nk_helmholtz_apply_host(basis.h, geom.h, float(lam), _ptr(host_in), _ptr(host_out), _stream(stream)))
+
+
+def probe_fp64_peak(iters=200):
+    tf, ms = _d(), _d()
+    _check(lib.nk_probe_fp64_peak(iters, C.byref(tf), C.byref(ms)))
+    return tf.value, ms.value
+
+
+def launch_count():
+    return lib.nk_launch_count()
+
+
+def version():
+    return lib.nk_version().decode()

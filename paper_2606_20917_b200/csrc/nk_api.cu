@@ -1,0 +1,546 @@
+// nk_api.cu -- the C-ABI of include/nk.h (layer B3), the dispatcher (B1), the geometry repack
+// kernels and the fp64 probe.  No torch types, no CPU fallback.
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/nk.h"
+#include "nk_host_tables.h"
+#include "nk_launch.h"
+
+#define NK_DECL(s, p) extern "C" const nk::InstInfo* NK_INST_NAME(s, p)();
+#define NK_LIST10(s) NK_DECL(s, 1) NK_DECL(s, 2) NK_DECL(s, 3) NK_DECL(s, 4) NK_DECL(s, 5) NK_DECL(s, 6) NK_DECL(s, 7) NK_DECL(s, 8)
+NK_LIST10(0) NK_DECL(0, 9) NK_DECL(0, 10)
+NK_LIST10(1)
+NK_LIST10(2)
+
+namespace {
+
+thread_local std::string g_err;
+long long g_launches = 0;
+std::mutex g_mutex;
+
+nk_status fail(nk_status s, const std::string& msg)
+{
+    g_err = msg;
+    return s;
+}
+nk_status cuda_fail(cudaError_t e, const char* what)
+{
+    g_err = std::string(what) + ": " + cudaGetErrorString(e);
+    return NK_ERR_CUDA;
+}
+
+typedef const nk::InstInfo* (*InstGetter)();
+const int kMaxP[3] = {10, 8, 8};
+InstGetter inst_getter(int shape, int P)
+{
+#define NK_G(s, p) NK_INST_NAME(s, p)
+    static const InstGetter tab[3][10] = {
+        {NK_G(0, 1), NK_G(0, 2), NK_G(0, 3), NK_G(0, 4), NK_G(0, 5), NK_G(0, 6), NK_G(0, 7), NK_G(0, 8), NK_G(0, 9), NK_G(0, 10)},
+        {NK_G(1, 1), NK_G(1, 2), NK_G(1, 3), NK_G(1, 4), NK_G(1, 5), NK_G(1, 6), NK_G(1, 7), NK_G(1, 8), nullptr, nullptr},
+        {NK_G(2, 1), NK_G(2, 2), NK_G(2, 3), NK_G(2, 4), NK_G(2, 5), NK_G(2, 6), NK_G(2, 7), NK_G(2, 8), nullptr, nullptr}};
+    if (shape < 0 || shape > 2 || P < 1 || P > kMaxP[shape]) return nullptr;
+    return tab[shape][P - 1];
+}
+
+int g_num_sms = 0;
+nk_status ensure_device()
+{
+    if (g_num_sms > 0) return NK_OK;
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice (no CUDA device: libnk has no CPU fallback)");
+    int n = 0;
+    e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+    g_num_sms = n;
+    return NK_OK;
+}
+
+} // namespace
+
+struct nk_basis {
+    nk::HostTables t;
+    const nk::InstInfo* inst = nullptr;
+    std::vector<double> tabs_flat; // DenseTabs<nm,Q> in declaration order
+    nk::SparseOff so;
+    std::vector<double> sp_d;
+    std::vector<int> sp_i;
+    mutable double* d_sp_d = nullptr;
+    mutable int* d_sp_i = nullptr;
+    mutable std::mutex mu;
+};
+
+struct nk_geom {
+    const nk_basis* b = nullptr;
+    int64_t nelem = 0, ngroups = 0;
+    int deformed = 0, E = 1;
+    double* d_metric = nullptr; // [group][7][npt][E]
+    double* d_factor = nullptr; // [group][10][npt][E]
+    double* d_stage_in = nullptr;
+    double* d_stage_out = nullptr;
+};
+
+// =========================== basis ===========================
+extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** out)
+{
+    if (!out) return fail(NK_ERR_INVALID_ARG, "nk_basis_create: out is NULL");
+    *out = nullptr;
+    if ((int)shape < 0 || (int)shape > 2 || P < 1 || Q < 2) return fail(NK_ERR_INVALID_ARG, "nk_basis_create: bad shape/P/Q");
+    InstGetter get = inst_getter((int)shape, P);
+    if (!get || Q != P + 2) {
+        char buf[160];
+        snprintf(buf, sizeof buf, "nk_basis_create: (shape=%d,P=%d,Q=%d) not instantiated (Q must be P+2; hex P<=10, tet/prism P<=8)", (int)shape, P, Q);
+        return fail(NK_ERR_UNSUPPORTED, buf);
+    }
+    nk_basis* b = new (std::nothrow) nk_basis;
+    if (!b) return fail(NK_ERR_ALLOC, "nk_basis_create: out of memory");
+    if (!nk::build_host_tables((int)shape, P, Q, b->t)) {
+        delete b;
+        return fail(NK_ERR_INVALID_ARG, "nk_basis_create: table construction failed");
+    }
+    b->inst = get();
+    const nk::HostTables& t = b->t;
+    const int nm = t.nm;
+    // DenseTabs: Ba[Q*nm], D[3][Q*Q], w[3][Q], aux[4][Q]
+    std::vector<double>& f = b->tabs_flat;
+    f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
+    for (int d = 0; d < 3; ++d) f.insert(f.end(), t.D[d].begin(), t.D[d].end());
+    for (int d = 0; d < 3; ++d) f.insert(f.end(), t.w[d].begin(), t.w[d].end());
+    for (int i = 0; i < Q; ++i) f.push_back(1.0 + t.z[0][i]);
+    for (int i = 0; i < Q; ++i) f.push_back(1.0 + t.z[1][i]);
+    for (int i = 0; i < Q; ++i) f.push_back(shape == NK_TET ? 1.0 / (1.0 - t.z[1][i]) : 0.0);
+    for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? 1.0 / (1.0 - t.z[2][i]) : 0.0);
+    (void)nm;
+    // sparse blob
+    nk::SparseOff& so = b->so;
+    std::memset(&so, 0, sizeof so);
+    if (shape != NK_HEX) {
+        so.tab3 = (int)b->sp_d.size();
+        b->sp_d.insert(b->sp_d.end(), t.tab3.begin(), t.tab3.end());
+        so.tab2 = (int)b->sp_d.size();
+        b->sp_d.insert(b->sp_d.end(), t.tab2.begin(), t.tab2.end());
+        auto put = [&](const std::vector<int>& v) {
+            const int off = (int)b->sp_i.size();
+            b->sp_i.insert(b->sp_i.end(), v.begin(), v.end());
+            return off;
+        };
+        so.s1f_start = put(t.s1f.start); so.s1f_src = put(t.s1f.src); so.s1f_row = put(t.s1f.row);
+        so.s1a_start = put(t.s1a.start); so.s1a_src = put(t.s1a.src); so.s1a_row = put(t.s1a.row);
+        so.s2f_start = put(t.s2f.start); so.s2f_src = put(t.s2f.src); so.s2f_row = put(t.s2f.row);
+        so.s2a_start = put(t.s2a.start); so.s2a_src = put(t.s2a.src); so.s2a_row = put(t.s2a.row);
+        if (b->sp_d.size() % 2) b->sp_d.push_back(0.0);
+        if (b->sp_i.size() % 2) b->sp_i.push_back(0);
+        so.ndoubles = (int)b->sp_d.size();
+        so.nints = (int)b->sp_i.size();
+    }
+    *out = b;
+    return NK_OK;
+}
+
+extern "C" nk_status nk_basis_destroy(nk_basis* b)
+{
+    if (!b) return NK_OK;
+    if (b->d_sp_d) cudaFree(b->d_sp_d);
+    if (b->d_sp_i) cudaFree(b->d_sp_i);
+    delete b;
+    return NK_OK;
+}
+
+extern "C" int nk_basis_num_modes(const nk_basis* b) { return b ? b->t.Nm : -1; }
+extern "C" int nk_basis_num_points(const nk_basis* b) { return b ? b->t.Nq : -1; }
+extern "C" int nk_basis_interleave(const nk_basis* b) { return b ? b->inst->E : -1; }
+
+extern "C" nk_status nk_basis_get_table(const nk_basis* b, int which, int dir, double* host_out, size_t cap, size_t* count)
+{
+    if (!b || dir < 0 || dir > 2) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_table: bad basis/dir");
+    const std::vector<double>* v = nullptr;
+    switch (which) {
+    case NK_TAB_NODES: v = &b->t.z[dir]; break;
+    case NK_TAB_WEIGHTS: v = &b->t.w[dir]; break;
+    case NK_TAB_DERIV: v = &b->t.D[dir]; break;
+    case NK_TAB_PSI: v = &b->t.psi[dir]; break;
+    default: return fail(NK_ERR_INVALID_ARG, "nk_basis_get_table: unknown table");
+    }
+    if (count) *count = v->size();
+    if (!host_out) return NK_OK;
+    if (cap < v->size()) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_table: capacity too small");
+    std::memcpy(host_out, v->data(), v->size() * sizeof(double));
+    return NK_OK;
+}
+
+extern "C" nk_status nk_basis_get_points(const nk_basis* b, double* xi_out, size_t cap)
+{
+    if (!b || !xi_out) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_points: NULL argument");
+    const nk::HostTables& t = b->t;
+    const int Q = t.Q;
+    if (cap < (size_t)3 * t.Nq) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_points: capacity too small");
+    for (int k = 0; k < Q; ++k)
+        for (int j = 0; j < Q; ++j)
+            for (int i = 0; i < Q; ++i) {
+                const double e1 = t.z[0][i], e2 = t.z[1][j], e3 = t.z[2][k];
+                double* x = xi_out + 3 * ((size_t)i + Q * (j + (size_t)Q * k));
+                x[0] = e1; x[1] = e2; x[2] = e3;
+                if (t.shape == nk::TET) {
+                    x[0] = 0.25 * (1.0 + e1) * (1.0 - e2) * (1.0 - e3) - 1.0;
+                    x[1] = 0.5 * (1.0 + e2) * (1.0 - e3) - 1.0;
+                } else if (t.shape == nk::PRISM) {
+                    x[0] = 0.5 * (1.0 + e1) * (1.0 - e3) - 1.0;
+                }
+            }
+    return NK_OK;
+}
+
+extern "C" int nk_basis_mode_index(const nk_basis* b, int p, int q, int r)
+{
+    return b ? nk::mode_index(b->t.shape, b->t.nm, p, q, r) : -1;
+}
+
+// =========================== geometry ===========================
+namespace {
+
+struct RepackTabs {
+    double z[3][12], w[3][12];
+    int shape, Q;
+};
+
+// chain matrix of Eq. 23 (A17) folded into the user's dxi/dx:  A'[l][i] = sum_j C[j][l] A[j][i]
+__device__ inline void fold_chain(int shape, const RepackTabs& rt, int i, int j, int k, double (&A)[9])
+{
+    if (shape == nk::K_TET) {
+        const double r2 = 1.0 / (1.0 - rt.z[1][j]), r3 = 1.0 / (1.0 - rt.z[2][k]);
+        const double c1 = 4.0 * r2 * r3, c2 = 2.0 * (1.0 + rt.z[0][i]) * r2 * r3, c3 = 2.0 * r3, c4 = (1.0 + rt.z[1][j]) * r3;
+        for (int x = 0; x < 3; ++x) {
+            const double a0 = A[0 + x], a1 = A[3 + x], a2 = A[6 + x];
+            A[0 + x] = c1 * a0 + c2 * (a1 + a2);
+            A[3 + x] = c3 * a1 + c4 * a2;
+        }
+    } else if (shape == nk::K_PRISM) {
+        const double r3 = 1.0 / (1.0 - rt.z[2][k]);
+        const double ca = 2.0 * r3, cb = (1.0 + rt.z[0][i]) * r3;
+        for (int x = 0; x < 3; ++x) A[0 + x] = ca * A[0 + x] + cb * A[6 + x];
+    }
+}
+
+// one thread per (group, point, e).  Deformed: quadrature weight and chain folded in.
+// Affine: npt = 1, plain factors (weights and chain are applied inside the kernels).
+__global__ void repack_kernel(const __grid_constant__ RepackTabs rt, const double* __restrict__ dxi_dx,
+                              const double* __restrict__ detJ, long long nelem, long long ngroups, int E, int deformed,
+                              double* __restrict__ metric, double* __restrict__ factor)
+{
+    const int Q = rt.Q;
+    const long long npt = deformed ? (long long)Q * Q * Q : 1;
+    const long long total = ngroups * npt * E;
+    for (long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x; t < total; t += (long long)gridDim.x * blockDim.x) {
+        const int e = (int)(t % E);
+        const long long n = (t / E) % npt, g = t / ((long long)E * npt);
+        const long long elem = g * E + e;
+        double A[9] = {0, 0, 0, 0, 0, 0, 0, 0, 0}, wJ = 0.0;
+        if (elem < nelem) {
+            const double* ap = dxi_dx + (elem * npt + n) * 9;
+            for (int c = 0; c < 9; ++c) A[c] = ap[c];
+            wJ = detJ[elem * npt + n];
+            if (deformed) {
+                const int k = (int)(n / (Q * Q)), j = (int)((n / Q) % Q), i = (int)(n % Q);
+                fold_chain(rt.shape, rt, i, j, k, A);
+                wJ *= rt.w[0][i] * rt.w[1][j] * rt.w[2][k];
+            }
+        }
+        double G[6];
+        G[0] = wJ * (A[0] * A[0] + A[1] * A[1] + A[2] * A[2]);
+        G[1] = wJ * (A[0] * A[3] + A[1] * A[4] + A[2] * A[5]);
+        G[2] = wJ * (A[0] * A[6] + A[1] * A[7] + A[2] * A[8]);
+        G[3] = wJ * (A[3] * A[3] + A[4] * A[4] + A[5] * A[5]);
+        G[4] = wJ * (A[3] * A[6] + A[4] * A[7] + A[5] * A[8]);
+        G[5] = wJ * (A[6] * A[6] + A[7] * A[7] + A[8] * A[8]);
+        for (int c = 0; c < 6; ++c) metric[((g * 7 + c) * npt + n) * E + e] = G[c];
+        metric[((g * 7 + 6) * npt + n) * E + e] = wJ;
+        for (int c = 0; c < 9; ++c) factor[((g * 10 + c) * npt + n) * E + e] = A[c];
+        factor[((g * 10 + 9) * npt + n) * E + e] = wJ;
+    }
+}
+
+nk_status ensure_sparse_on_device(const nk_basis* b)
+{
+    if (b->t.shape == nk::HEX || b->d_sp_d) return NK_OK;
+    std::lock_guard<std::mutex> lk(b->mu);
+    if (b->d_sp_d) return NK_OK;
+    double* dd = nullptr;
+    int* di = nullptr;
+    cudaError_t e = cudaMalloc(&dd, b->sp_d.size() * sizeof(double));
+    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(sparse tables)");
+    e = cudaMalloc(&di, b->sp_i.size() * sizeof(int));
+    if (e != cudaSuccess) { cudaFree(dd); return cuda_fail(e, "cudaMalloc(sparse tables)"); }
+    e = cudaMemcpy(dd, b->sp_d.data(), b->sp_d.size() * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess) e = cudaMemcpy(di, b->sp_i.data(), b->sp_i.size() * sizeof(int), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) { cudaFree(dd); cudaFree(di); return cuda_fail(e, "cudaMemcpy(sparse tables)"); }
+    b->d_sp_i = di;
+    b->d_sp_d = dd;
+    return NK_OK;
+}
+
+} // namespace
+
+extern "C" nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
+                                    const double* detJ, int on_device, void* stream, nk_geom** out)
+{
+    if (!out) return fail(NK_ERR_INVALID_ARG, "nk_geom_upload: out is NULL");
+    *out = nullptr;
+    if (!b || nelem < 0 || (nelem > 0 && (!dxi_dx || !detJ))) return fail(NK_ERR_INVALID_ARG, "nk_geom_upload: bad arguments");
+    nk_status st = ensure_device();
+    if (st != NK_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    nk_geom* g = new (std::nothrow) nk_geom;
+    if (!g) return fail(NK_ERR_ALLOC, "nk_geom_upload: out of memory");
+    g->b = b;
+    g->nelem = nelem;
+    g->deformed = deformed ? 1 : 0;
+    g->E = b->inst->E;
+    g->ngroups = (nelem + g->E - 1) / g->E;
+    *out = g;
+    if (nelem == 0) return NK_OK;
+    const long long npt = g->deformed ? b->t.Nq : 1;
+    const size_t slots = (size_t)g->ngroups * npt * g->E;
+    cudaError_t e = cudaMalloc(&g->d_metric, slots * 7 * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&g->d_factor, slots * 10 * sizeof(double));
+    if (e != cudaSuccess) {
+        nk_geom_destroy(g);
+        *out = nullptr;
+        g_err = std::string("nk_geom_upload: cudaMalloc: ") + cudaGetErrorString(e);
+        return NK_ERR_ALLOC;
+    }
+    const double *dA = dxi_dx, *dJ = detJ;
+    double *tA = nullptr, *tJ = nullptr;
+    if (!on_device) {
+        const size_t nA = (size_t)nelem * npt * 9, nJ = (size_t)nelem * npt;
+        e = cudaMalloc(&tA, nA * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc(&tJ, nJ * sizeof(double));
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tA, dxi_dx, nA * sizeof(double), cudaMemcpyHostToDevice, s);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(tJ, detJ, nJ * sizeof(double), cudaMemcpyHostToDevice, s);
+        if (e != cudaSuccess) {
+            cudaFree(tA); cudaFree(tJ);
+            nk_geom_destroy(g);
+            *out = nullptr;
+            return cuda_fail(e, "nk_geom_upload: staging copy");
+        }
+        dA = tA;
+        dJ = tJ;
+    }
+    RepackTabs rt;
+    std::memset(&rt, 0, sizeof rt);
+    rt.shape = b->t.shape;
+    rt.Q = b->t.Q;
+    for (int d = 0; d < 3; ++d)
+        for (int i = 0; i < b->t.Q; ++i) {
+            rt.z[d][i] = b->t.z[d][i];
+            rt.w[d][i] = b->t.w[d][i];
+        }
+    const int threads = 256;
+    long long blocks = ((long long)slots + threads - 1) / threads;
+    if (blocks > 148LL * 32) blocks = 148LL * 32;
+    repack_kernel<<<(int)blocks, threads, 0, s>>>(rt, dA, dJ, nelem, g->ngroups, g->E, g->deformed, g->d_metric, g->d_factor);
+    e = cudaGetLastError();
+    { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
+    if (!on_device) {
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        cudaFree(tA);
+        cudaFree(tJ);
+    }
+    if (e != cudaSuccess) {
+        nk_geom_destroy(g);
+        *out = nullptr;
+        return cuda_fail(e, "nk_geom_upload: repack");
+    }
+    return NK_OK;
+}
+
+extern "C" nk_status nk_geom_destroy(nk_geom* g)
+{
+    if (!g) return NK_OK;
+    if (g->d_metric) cudaFree(g->d_metric);
+    if (g->d_factor) cudaFree(g->d_factor);
+    if (g->d_stage_in) cudaFree(g->d_stage_in);
+    if (g->d_stage_out) cudaFree(g->d_stage_out);
+    delete g;
+    return NK_OK;
+}
+
+extern "C" int64_t nk_geom_num_elements(const nk_geom* g) { return g ? g->nelem : -1; }
+
+// =========================== operators ===========================
+namespace {
+
+nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, int64_t nelem, const double* in0,
+                 const double* in1, const double* in2, double* out0, double* out1, double* out2, double lambda,
+                 void* stream)
+{
+    if (!b) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": basis is NULL");
+    if (op != nk::OP_BWD) {
+        if (!g) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": geom is NULL");
+        if (g->b != b && (g->b->t.shape != b->t.shape || g->b->t.P != b->t.P || g->b->t.Q != b->t.Q))
+            return fail(NK_ERR_SHAPE_MISMATCH, std::string(name) + ": geom was uploaded for another basis");
+        nelem = g->nelem;
+    }
+    if (nelem < 0) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": nelem < 0");
+    if (nelem == 0) return NK_OK;
+    const bool need_in0 = (op != nk::OP_IPDERIV);
+    if ((need_in0 && !in0) || (op != nk::OP_PHYSDERIV && !out0))
+        return fail(NK_ERR_INVALID_ARG, std::string(name) + ": NULL field pointer");
+    if (in0 && (in0 == out0)) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": in and out alias");
+    nk_status st = ensure_device();
+    if (st != NK_OK) return st;
+    st = ensure_sparse_on_device(b);
+    if (st != NK_OK) return st;
+    const int E = b->inst->E;
+    nk::KArgs a;
+    a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
+    a.out[0] = out0; a.out[1] = out1; a.out[2] = out2;
+    a.geom = nullptr;
+    int def = 0;
+    if (g) {
+        def = g->deformed;
+        a.geom = (op == nk::OP_PHYSDERIV || op == nk::OP_IPDERIV) ? g->d_factor : g->d_metric;
+    }
+    a.sparse_d = b->d_sp_d;
+    a.sparse_i = b->d_sp_i;
+    a.lambda = lambda;
+    a.nelem = nelem;
+    const int64_t ngroups = (nelem + E - 1) / E;
+    if (ngroups > 0x7fffffffLL) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": too many elements");
+    a.ngroups = (int)ngroups;
+    cudaError_t e = b->inst->fn[def][op](b->tabs_flat.data(), b->so, a, g_num_sms, (cudaStream_t)stream);
+    if (e != cudaSuccess) return cuda_fail(e, name);
+    { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
+    return NK_OK;
+}
+
+} // namespace
+
+extern "C" nk_status nk_bwdtrans(const nk_basis* b, int64_t nelem, const double* coeffs, double* phys, void* stream)
+{
+    return run_op(nk::OP_BWD, "nk_bwdtrans", b, nullptr, nelem, coeffs, nullptr, nullptr, phys, nullptr, nullptr, 0.0, stream);
+}
+extern "C" nk_status nk_iprod(const nk_basis* b, const nk_geom* g, const double* phys, double* coeffs, void* stream)
+{
+    return run_op(nk::OP_IPROD, "nk_iprod", b, g, 0, phys, nullptr, nullptr, coeffs, nullptr, nullptr, 0.0, stream);
+}
+extern "C" nk_status nk_physderiv(const nk_basis* b, const nk_geom* g, const double* phys, double* d0, double* d1,
+                                  double* d2, void* stream)
+{
+    return run_op(nk::OP_PHYSDERIV, "nk_physderiv", b, g, 0, phys, nullptr, nullptr, d0, d1, d2, 0.0, stream);
+}
+extern "C" nk_status nk_iprod_deriv(const nk_basis* b, const nk_geom* g, const double* g0, const double* g1,
+                                    const double* g2, double* coeffs, void* stream)
+{
+    return run_op(nk::OP_IPDERIV, "nk_iprod_deriv", b, g, 0, g0, g1, g2, coeffs, nullptr, nullptr, 0.0, stream);
+}
+extern "C" nk_status nk_mass_apply(const nk_basis* b, const nk_geom* g, const double* in, double* out, void* stream)
+{
+    return run_op(nk::OP_MASS, "nk_mass_apply", b, g, 0, in, nullptr, nullptr, out, nullptr, nullptr, 0.0, stream);
+}
+extern "C" nk_status nk_laplacian_apply(const nk_basis* b, const nk_geom* g, const double* in, double* out, void* stream)
+{
+    return run_op(nk::OP_LAP, "nk_laplacian_apply", b, g, 0, in, nullptr, nullptr, out, nullptr, nullptr, 0.0, stream);
+}
+extern "C" nk_status nk_helmholtz_apply(const nk_basis* b, const nk_geom* g, double lambda, const double* in,
+                                        double* out, void* stream)
+{
+    return run_op(nk::OP_HELM, "nk_helmholtz_apply", b, g, 0, in, nullptr, nullptr, out, nullptr, nullptr, lambda, stream);
+}
+
+extern "C" nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double lambda, void* stream)
+{
+    if (nblocks < 0 || (nblocks > 0 && !blocks)) return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_blocks: bad arguments");
+    for (int i = 0; i < nblocks; ++i) {
+        nk_status st = nk_helmholtz_apply(blocks[i].basis, blocks[i].geom, lambda, blocks[i].in, blocks[i].out, stream);
+        if (st != NK_OK) return st;
+    }
+    return NK_OK;
+}
+
+extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* gc, double lambda, const double* host_in,
+                                             double* host_out, void* stream)
+{
+    if (!b || !gc || !host_in || !host_out) return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_host: NULL argument");
+    nk_geom* g = const_cast<nk_geom*>(gc);
+    if (g->nelem == 0) return NK_OK;
+    const size_t bytes = (size_t)g->nelem * b->t.Nm * sizeof(double);
+    cudaError_t e = cudaSuccess;
+    if (!g->d_stage_in) {
+        e = cudaMalloc(&g->d_stage_in, bytes);
+        if (e == cudaSuccess) e = cudaMalloc(&g->d_stage_out, bytes);
+        if (e != cudaSuccess) { g_err = "nk_helmholtz_apply_host: cudaMalloc failed"; return NK_ERR_ALLOC; }
+    }
+    cudaStream_t s = (cudaStream_t)stream;
+    e = cudaMemcpyAsync(g->d_stage_in, host_in, bytes, cudaMemcpyHostToDevice, s);
+    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: H2D");
+    nk_status st = nk_helmholtz_apply(b, g, lambda, g->d_stage_in, g->d_stage_out, stream);
+    if (st != NK_OK) return st;
+    e = cudaMemcpyAsync(host_out, g->d_stage_out, bytes, cudaMemcpyDeviceToHost, s);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: D2H");
+    return NK_OK;
+}
+
+// =========================== diagnostics ===========================
+namespace {
+__global__ void __launch_bounds__(256) dfma_probe(int iters, double x, double y, double* sink)
+{
+    double acc[8];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) acc[c] = threadIdx.x * 1e-9 + c;
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 512; ++u) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) acc[c] = fma(acc[c], x, y);
+        }
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) s += acc[c];
+    if (s == 123.456) sink[0] = s;
+}
+} // namespace
+
+extern "C" nk_status nk_probe_fp64_peak(int iters, double* tflops, double* ms_out)
+{
+    if (iters < 1 || !tflops) return fail(NK_ERR_INVALID_ARG, "nk_probe_fp64_peak: bad arguments");
+    nk_status st = ensure_device();
+    if (st != NK_OK) return st;
+    double* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, sizeof(double));
+    if (e != cudaSuccess) return cuda_fail(e, "nk_probe_fp64_peak: cudaMalloc");
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    const int blocks = g_num_sms * 8, threads = 256;
+    dfma_probe<<<blocks, threads>>>(1, 0.999999, 1e-9, sink); // warm-up
+    cudaEventRecord(t0);
+    dfma_probe<<<blocks, threads>>>(iters, 0.999999, 1e-9, sink);
+    cudaEventRecord(t1);
+    e = cudaEventSynchronize(t1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, t0, t1);
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(sink);
+    { std::lock_guard<std::mutex> lk(g_mutex); g_launches += 2; }
+    if (e != cudaSuccess) return cuda_fail(e, "nk_probe_fp64_peak");
+    const double flops = 2.0 * 4096.0 * iters * (double)blocks * threads;
+    *tflops = flops / (ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = ms;
+    return NK_OK;
+}
+
+extern "C" int64_t nk_launch_count(void)
+{
+    std::lock_guard<std::mutex> lk(g_mutex);
+    return g_launches;
+}
+extern "C" const char* nk_last_error(void) { return g_err.c_str(); }
+extern "C" const char* nk_version(void) { return "libnk 0.1 (sm_100a)"; }

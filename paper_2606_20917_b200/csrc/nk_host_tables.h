@@ -1,0 +1,45 @@
+// nk_host_tables.h -- host precompute of the 1-D ingredients of the modified
+// C0 basis and its quadrature (layer B2).  Plain C++; no CUDA; shares nothing
+// with oracle/.  Citations: P:<n> = paper line, A<n> = DESIGN.md section 3.
+#pragma once
+#include <vector>
+
+namespace nk {
+
+enum { HEX = 0, TET = 1, PRISM = 2 };
+
+// A sparse "line stage": output o = sum over entries en in [start[o], start[o+1]) of
+// input[src[en]] (x) table row row[en].  These are the index arrays that replace the
+// triangular loop nests of Eq. 17 / Eq. 21 (cf. the index arrays of P:302)
+// and carry the top-vertex / top-edge corrections of A8 as ordinary entries.
+struct SparseStage {
+    std::vector<int> start, src, row;
+};
+
+struct HostTables {
+    int shape = 0, P = 0, Q = 0, nm = 0, Nm = 0, Nq = 0, npair = 0;
+    std::vector<double> z[3], w[3]; // nodes; weights with the collapse Jacobian folded in (A16)
+    std::vector<double> D[3];       // D[d][i*Q + r] = h_r'(z_i)   (Eq. 22)
+    int ncol[3] = {0, 0, 0};
+    std::vector<double> psi[3];     // psi[d][i*ncol[d] + col]   (point-major, see nk.h NK_TAB_PSI)
+    // simplices only
+    int n1 = 0;                     // number of (p,q) lines after the r-sum
+    std::vector<double> tab3;       // [row][k]  psi^b_{s,r}(z3_k), row = pair(s,r)
+    std::vector<double> tab2;       // [row][j]  psi^b_{p,q}(z2_j), row = pair(p,q)   (tet)
+    SparseStage s1f, s1a, s2f, s2a;
+};
+
+// Jacobi polynomial P_n^{a,b}(x) (A7)
+double jacobi(int n, double a, double b, double x);
+// modified principal functions (A7)
+double psi_a(int p, double z);
+double psi_b(int i, int j, double z);
+
+int pair_index(int nm, int a, int b);                   // sum_{c<a}(nm-c) + b
+int mode_index(int shape, int nm, int p, int q, int r); // Eq. 18 (A3); -1 if not a mode
+int num_modes(int shape, int nm);
+
+// returns false if (shape,P,Q) is malformed (P<1, Q<2)
+bool build_host_tables(int shape, int P, int Q, HostTables& t);
+
+} // namespace nk

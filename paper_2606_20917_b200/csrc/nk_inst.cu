@@ -1,0 +1,55 @@
+// nk_inst.cu -- explicit instantiation of nk_kernel for ONE (shape, P), Q = P+2; compiled once per
+// pair with -DNK_SHAPE=<0|1|2> -DNK_P=<order>.  Compile-time specialisation over (shape, P, Q,
+// deformed, op) replaces the paper's JIT (north_star).
+#include <cstring>
+
+#include "nk_kernel_body.cuh"
+#include "nk_launch.h"
+
+#ifndef NK_SHAPE
+#error "compile with -DNK_SHAPE and -DNK_P"
+#endif
+
+namespace nk {
+
+template <int SHAPE, int P, int DEF, int OP>
+static cudaError_t launch(const double* tabs_flat, const SparseOff& so, const KArgs& a, int num_sms, cudaStream_t stream)
+{
+    using T = Tune<SHAPE, P>;
+    static int blocks_per_sm = 0;
+    DenseTabs<P + 1, P + 2> tabs;
+    std::memcpy(&tabs, tabs_flat, sizeof(tabs));
+    const size_t smem = T::smem_grid + (SHAPE != K_HEX ? (size_t)so.ndoubles * 8 + (size_t)so.nints * 4 : 0);
+    auto kern = nk_kernel<SHAPE, P, DEF, OP>;
+    if (blocks_per_sm == 0) {
+        cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+        if (err != cudaSuccess) return err;
+        int bps = 0;
+        err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, T::NT, smem);
+        if (err != cudaSuccess) return err;
+        blocks_per_sm = bps < 1 ? 1 : bps;
+    }
+    if (a.ngroups <= 0) return cudaSuccess;
+    const long long cap = (long long)num_sms * blocks_per_sm;
+    const int grid = (int)(a.ngroups < cap ? a.ngroups : cap);
+    kern<<<grid, T::NT, smem, stream>>>(tabs, so, a);
+    return cudaGetLastError();
+}
+
+#define NK_ROW(DEF)                                                                                     \
+    {                                                                                                   \
+        launch<NK_SHAPE, NK_P, DEF, OP_BWD>, launch<NK_SHAPE, NK_P, DEF, OP_IPROD>,                     \
+            launch<NK_SHAPE, NK_P, DEF, OP_PHYSDERIV>, launch<NK_SHAPE, NK_P, DEF, OP_IPDERIV>,         \
+            launch<NK_SHAPE, NK_P, DEF, OP_MASS>, launch<NK_SHAPE, NK_P, DEF, OP_LAP>,                  \
+            launch<NK_SHAPE, NK_P, DEF, OP_HELM>                                                        \
+    }
+
+} // namespace nk
+
+extern "C" const nk::InstInfo* NK_INST_NAME(NK_SHAPE, NK_P)()
+{
+    using namespace nk;
+    using T = nk::Tune<NK_SHAPE, NK_P>;
+    static const nk::InstInfo info = {NK_SHAPE, NK_P, NK_P + 2, T::E, T::NT, T::MINB, T::smem_grid, {NK_ROW(0), NK_ROW(1)}};
+    return &info;
+}

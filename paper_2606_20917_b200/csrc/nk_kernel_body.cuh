@@ -1,0 +1,153 @@
+// nk_kernel_body.cuh -- the kernel template itself (see nk_kernels.cuh for the design).
+// Stage names follow SURVEY 8(a): a1 load, a2 BwdTrans (S1,S2,S3), a3 standard derivative
+// (passes A,B,C), a4 chain, a5 geometry, a6 chain^T, a7 D^T (passes C,D,E), a8 IProduct
+// (S3^T,S2^T,S1^T), a9 store.
+#pragma once
+#include "nk_kernels.cuh"
+
+namespace nk {
+
+// chain of Eq. 23 with the factors of A17 at one point: (d/d eta) -> (d/d xi)
+template <int SHAPE>
+__device__ __forceinline__ void chain_fwd(double c1, double c2, double c3, double c4, double& a, double& b, double& c)
+{
+    if constexpr (SHAPE == K_TET) {
+        const double t = c2 * a;
+        const double x3 = fma(c4, b, t) + c;
+        b = fma(c3, b, t);
+        a = c1 * a;
+        c = x3;
+    } else if constexpr (SHAPE == K_PRISM) {
+        c = fma(c2, a, c);
+        a = c1 * a;
+    }
+}
+// its transpose: (xi-components) -> (eta-components)
+template <int SHAPE>
+__device__ __forceinline__ void chain_adj(double c1, double c2, double c3, double c4, double& a, double& b, double& c)
+{
+    if constexpr (SHAPE == K_TET) {
+        a = fma(c1, a, c2 * (b + c));
+        b = fma(c3, b, c4 * c);
+    } else if constexpr (SHAPE == K_PRISM) {
+        a = fma(c1, a, c2 * c);
+    }
+}
+
+template <int SHAPE, int P, int DEF, int OP>
+__global__ void __launch_bounds__(Tune<SHAPE, P>::NT, Tune<SHAPE, P>::MINB)
+nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_constant__ SparseOff so,
+          const __grid_constant__ KArgs a)
+{
+    using T = Tune<SHAPE, P>;
+    constexpr int NM = P + 1, Q = P + 2, E = T::E, LS = T::LS, LQ = T::LQ;
+    constexpr int NQ = Q * Q * Q, NQP = T::NQP, NMODES = k_num_modes(SHAPE, NM);
+    constexpr bool IN_COEFF = (OP == OP_BWD || OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);
+    constexpr bool OUT_COEFF = (OP != OP_BWD && OP != OP_PHYSDERIV);
+    constexpr bool FWD_D = (OP == OP_PHYSDERIV || OP == OP_LAP || OP == OP_HELM);
+    constexpr bool ADJ_D = (OP == OP_IPDERIV || OP == OP_LAP || OP == OP_HELM);
+    constexpr bool SP1 = (SHAPE != K_HEX), SP2 = (SHAPE == K_TET);
+    constexpr bool CHAIN = (SHAPE != K_HEX) && !DEF; // deformed simplices: chain folded at upload
+    constexpr int N1 = SP2 ? NM * (NM + 1) / 2 : NM * NM;
+    constexpr int NCG = (OP == OP_PHYSDERIV || OP == OP_IPDERIV) ? 10 : 7;
+
+    extern __shared__ double sm[];
+    double* __restrict__ X = sm;
+    double* __restrict__ Y = sm + (size_t)NQP * E;
+    double* __restrict__ Z = sm + (size_t)2 * NQP * E;
+    double* sd = sm + (size_t)3 * NQP * E;
+    int* si = reinterpret_cast<int*>(sd + so.ndoubles);
+
+    const int tid = threadIdx.x;
+    const int e = tid % E, slot = tid / E;
+#define GIDX(i, j, k) (((i) + LQ * ((j) + Q * (k))) * E + e)
+
+    if constexpr (SP1) { // stage the sparse tables once per block
+        for (int t = tid; t < so.ndoubles; t += T::NT) sd[t] = __ldg(a.sparse_d + t);
+        for (int t = tid; t < so.nints; t += T::NT) si[t] = __ldg(a.sparse_i + t);
+        __syncthreads();
+    }
+    const double* tab3 = sd + so.tab3;
+    const double* tab2 = sd + so.tab2;
+
+    for (int g = blockIdx.x; g < a.ngroups; g += gridDim.x) {
+        const long long elem = (long long)g * E + e;
+        const bool valid = elem < a.nelem;
+        const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
+        (void)geo;
+
+        // ================= input side =================
+        if constexpr (IN_COEFF) {
+            // a1: coefficients -> Y as C[m]
+            const double* __restrict__ src = a.in[0] + elem * NMODES;
+            for (int m = slot; m < NMODES; m += LS) Y[m * E + e] = valid ? __ldg(src + m) : 0.0;
+            __syncthreads();
+            // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
+            if constexpr (!SP1) {
+                for (int l = slot; l < NM * NM; l += LS) {
+                    double c[NM];
+                    NK_UNROLL for (int r = 0; r < NM; ++r) c[r] = Y[(l * NM + r) * E + e];
+                    NK_UNROLL for (int k = 0; k < Q; ++k) {
+                        double acc = 0.0;
+                        NK_UNROLL for (int r = 0; r < NM; ++r) acc = fma(tabs.Ba[k * NM + r], c[r], acc);
+                        Z[(l * Q + k) * E + e] = acc;
+                    }
+                }
+            } else {
+                const int* st = si + so.s1f_start;
+                const int* sr = si + so.s1f_src;
+                const int* rw = si + so.s1f_row;
+                for (int l = slot; l < N1; l += LS) {
+                    double acc[Q];
+                    NK_UNROLL for (int k = 0; k < Q; ++k) acc[k] = 0.0;
+                    const int e1 = st[l + 1];
+                    for (int en = st[l]; en < e1; ++en) {
+                        const double c = Y[sr[en] * E + e];
+                        const double* tb = tab3 + rw[en] * Q;
+                        NK_UNROLL for (int k = 0; k < Q; ++k) acc[k] = fma(c, tb[k], acc[k]);
+                    }
+                    NK_UNROLL for (int k = 0; k < Q; ++k) Z[(l * Q + k) * E + e] = acc[k];
+                }
+            }
+            __syncthreads();
+            // a2/S2: sum over q:  T1 -> T2[p][j][k] in X
+            if constexpr (!SP2) {
+                for (int l = slot; l < NM * Q; l += LS) {
+                    const int p = l / Q, k = l - p * Q;
+                    double c[NM];
+                    NK_UNROLL for (int q = 0; q < NM; ++q) c[q] = Z[((p * NM + q) * Q + k) * E + e];
+                    NK_UNROLL for (int j = 0; j < Q; ++j) {
+                        double acc = 0.0;
+                        NK_UNROLL for (int q = 0; q < NM; ++q) acc = fma(tabs.Ba[j * NM + q], c[q], acc);
+                        X[((p * Q + j) * Q + k) * E + e] = acc;
+                    }
+                }
+            } else {
+                const int* st = si + so.s2f_start;
+                const int* sr = si + so.s2f_src;
+                const int* rw = si + so.s2f_row;
+                for (int l = slot; l < NM * Q; l += LS) {
+                    const int p = l / Q, k = l - p * Q;
+                    double acc[Q];
+                    NK_UNROLL for (int j = 0; j < Q; ++j) acc[j] = 0.0;
+                    const int e1 = st[p + 1];
+                    for (int en = st[p]; en < e1; ++en) {
+                        const double c = Z[(sr[en] * Q + k) * E + e];
+                        const double* tb = tab2 + rw[en] * Q;
+                        NK_UNROLL for (int j = 0; j < Q; ++j) acc[j] = fma(c, tb[j], acc[j]);
+                    }
+                    NK_UNROLL for (int j = 0; j < Q; ++j) X[((p * Q + j) * Q + k) * E + e] = acc[j];
+                }
+            }
+            __syncthreads();
+#include "nk_stage_s3.inc"
+        } else {
+#include "nk_stage_physin.inc"
+        }
+#include "nk_stage_mid.inc"
+#include "nk_stage_out.inc"
+    }
+#undef GIDX
+}
+
+} // namespace nk

@@ -1,0 +1,98 @@
+// nk_kernels.cuh -- sm_100a kernels of libnk (layer B0).
+//
+// One kernel template, nk_kernel<SHAPE,P,DEF,OP>, covers every operator of nk.h.
+// Design:
+//   * a thread block works on a GROUP of E elements at a time; all on-chip arrays are
+//     element-interleaved, index = idx*E + e, thread = (e = tid % E, slot = tid / E).
+//     A half-warp therefore touches E consecutive doubles per line: shared-memory accesses
+//     are conflict-free by construction and the geometry stream (stored in the same
+//     interleaved order) is read as fully coalesced 256-byte warp loads.
+//   * every tensor contraction is "one thread per quadrature LINE": the thread pulls one
+//     line of one element into registers and contracts it with a 1-D matrix whose entries
+//     are compile-time-indexed kernel parameters, i.e. constant-bank operands of DFMA --
+//     no shared-memory traffic for the basis / derivative matrices (Eq. 16, 20, 22).
+//   * the simplex contractions with triangular bounds (Eq. 17, 21) run from host-built
+//     index arrays staged once per block in shared memory; the C0 corrections
+//     of A8 are ordinary entries of those arrays.
+//   * the Helmholtz chain (a1..a9 of SURVEY 8(a)) is fused: three shared arrays X, Y, Z of
+//     Q^3*E doubles are reused by a static plan (cf. the buffer-reuse pass);
+//     quadrature-point data never goes to HBM.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+namespace nk {
+
+enum { K_HEX = 0, K_TET = 1, K_PRISM = 2 };
+enum { OP_BWD = 0, OP_IPROD, OP_PHYSDERIV, OP_IPDERIV, OP_MASS, OP_LAP, OP_HELM, OP_COUNT };
+
+__host__ __device__ constexpr int k_num_modes(int shape, int nm)
+{
+    return shape == K_HEX ? nm * nm * nm : shape == K_TET ? nm * (nm + 1) * (nm + 2) / 6 : nm * nm * (nm + 1) / 2;
+}
+
+// ---- launch configuration per (shape, P); Q = P+2 --------------------------------------
+// E  = elements per group (interleave width), LS = line slots, threads = E*LS,
+// LQ = padded length of an i-line in the point arrays (odd when E < 16 so that the
+//      (j,k)-line pass stays bank-conflict-free), MINB = blocks per SM asked of ptxas.
+template <int SHAPE, int P>
+struct Tune {
+    static constexpr int Q = P + 2;
+#if defined(NK_TUNE_E)
+    static constexpr int E = NK_TUNE_E;
+#else
+    static constexpr int E = Q <= 4 ? 32 : Q <= 5 ? 16 : Q <= 8 ? 8 : Q <= 10 ? 4 : 2;
+#endif
+    static constexpr int LQ = (E >= 16) ? Q : (Q | 1);
+    static constexpr int NQP = LQ * Q * Q;
+#if defined(NK_TUNE_LS)
+    static constexpr int LS = NK_TUNE_LS;
+#else
+    static constexpr int LS_full = Q * Q;
+    // aim at 128..320 threads
+    static constexpr int LS = (E * LS_full <= 320) ? LS_full : (E * ((LS_full + 1) / 2) <= 320) ? (LS_full + 1) / 2
+                              : (E * ((LS_full + 2) / 3) <= 320) ? (LS_full + 2) / 3 : (LS_full + 3) / 4;
+#endif
+    static constexpr int NT = E * LS;
+    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
+#if defined(NK_TUNE_MINB)
+    static constexpr int MINB = NK_TUNE_MINB;
+#else
+    static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + 2048));
+    static constexpr int MINB_reg = 65536 / (NT * 104);
+    static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
+#endif
+};
+
+// ---- kernel parameters (constant bank) -------------------------------------------------
+template <int NM, int Q>
+struct DenseTabs {
+    double Ba[Q * NM];   // [i][p]  psi^a_p at the GLL points (directions whose basis is psi^a)
+    double D[3][Q * Q];  // [d][i][r]  D^(d)[i][r] = h_r'(z_i)   (Eq. 22)
+    double w[3][Q];      // 1-D weights (collapse Jacobian folded in, A16)
+    double aux[4][Q];    // chain helpers (A17): 1+z1, 1+z2, 1/(1-z2), 1/(1-z3)
+};
+
+struct SparseOff {       // offsets into the sparse blob (doubles first, then ints)
+    int ndoubles, nints;
+    int tab3, tab2;                                  // double offsets
+    int s1f_start, s1f_src, s1f_row;                 // int offsets
+    int s1a_start, s1a_src, s1a_row;
+    int s2f_start, s2f_src, s2f_row;
+    int s2a_start, s2a_src, s2a_row;
+};
+
+struct KArgs {
+    const double* in[3];
+    double* out[3];
+    const double* geom;      // metric stream (7 comps) or factor stream (10 comps), see nk_api.cu
+    const double* sparse_d;  // device copy of the sparse blob
+    const int* sparse_i;
+    double lambda;
+    long long nelem;
+    int ngroups;
+};
+
+#define NK_UNROLL _Pragma("unroll")
+
+} // namespace nk

@@ -1,0 +1,21 @@
+// nk_launch.h -- type-erased launch table shared by the per-(shape,P) instantiation units
+// (nk_inst.cu, compiled once per pair) and the dispatcher in nk_api.cu (layer B1).
+#pragma once
+#include "nk_kernels.cuh"
+
+namespace nk {
+
+// tabs_flat: the doubles of DenseTabs<P+1,P+2> in declaration order.
+typedef cudaError_t (*LaunchFn)(const double* tabs_flat, const SparseOff& so, const KArgs& a, int num_sms,
+                                cudaStream_t stream);
+
+struct InstInfo {
+    int shape, P, Q, E, threads, blocks_per_sm_hint;
+    size_t smem_grid;
+    LaunchFn fn[2][OP_COUNT]; // [deformed][op]
+};
+
+} // namespace nk
+
+#define NK_INST_NAME2(s, p) nk_inst_##s##_##p
+#define NK_INST_NAME(s, p) NK_INST_NAME2(s, p)

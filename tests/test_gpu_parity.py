@@ -1,0 +1,167 @@
+"""GPU parity: every operator of include/nk.h, called through the C-ABI binding, against the
+plain CPU oracle on the same seeded inputs.  Gate (north_star; A18): normwise relative
+error per element <= 1e-12 in fp64."""
+import numpy as np
+import pytest
+import torch
+
+import nk_cases as K
+from oracle import nk_oracle as o
+from workloads import synthetic as wl
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def nk():
+    import paper_2606_20917_b200 as nk
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return nk
+
+
+def run_case(nk, shape, P, n, deformed, ops, lam=1.0, take=None, seed=wl.SEED0, zhi=None):
+    el = K.element(shape, P)
+    A, J = K.geometry(shape, P, n, deformed, take=take, zhi=zhi)
+    ne = J.shape[0]
+    basis = nk.Basis(shape, P)
+    assert basis.num_modes == el.Nm and basis.num_points == el.Nq
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), deformed)
+    errs = {}
+    for op in ops:
+        x = K.make_input(op, seed, ne, el)
+        ref = K.oracle_op(op, el, A, J, lam, x)
+        got = K.gpu_op(nk, op, basis, geom, lam, x)
+        assert np.isfinite(got).all(), (op, "non-finite output")
+        errs[op] = K.op_err(op, got, ref)
+    bad = {k: v for k, v in errs.items() if not v <= TOL}
+    assert not bad, "shape %d P %d def %d: %r" % (shape, P, deformed, errs)
+    return errs
+
+
+def test_config1_hex_affine_P3_64_elements(nk):
+    """BASELINE config 1 in full: BwdTrans, IProductWRTBase, Helmholtz lambda=1 (plus the rest)."""
+    run_case(nk, o.HEX, 3, 4, False, K.OPS, lam=1.0, seed=wl.SEED0 + 1)
+
+
+@pytest.mark.parametrize("shape", [o.HEX, o.TET, o.PRISM])
+@pytest.mark.parametrize("deformed", [False, True])
+def test_all_ops_P4_ragged(nk, shape, deformed):
+    """several groups plus a ragged tail (nelem not a multiple of the interleave width)."""
+    full = K.mesh(shape, 3)[0].shape[0]
+    take = torch.arange(full - 5)
+    run_case(nk, shape, 4, 3, deformed, K.OPS, lam=1.0, take=take, seed=wl.SEED0 + 2)
+
+
+@pytest.mark.parametrize("P", range(1, 11))
+def test_config4_hex_psweep_mass_laplacian(nk, P):
+    run_case(nk, o.HEX, P, 3 if P < 8 else 2, False, ("mass", "laplacian"), seed=wl.SEED0 + 4)
+
+
+@pytest.mark.parametrize("P", range(1, 11))
+def test_hex_deformed_all_orders(nk, P):
+    run_case(nk, o.HEX, P, 2, True, ("helmholtz", "physderiv", "iprod_deriv"), lam=0.7, seed=wl.SEED0 + 4)
+
+
+@pytest.mark.parametrize("shape", [o.TET, o.PRISM])
+@pytest.mark.parametrize("P", range(1, 9))
+def test_simplex_all_orders(nk, shape, P):
+    for deformed in (False, True):
+        run_case(nk, shape, P, 2, deformed, ("bwdtrans", "iprod", "helmholtz", "physderiv", "iprod_deriv"),
+                 lam=10.0, seed=wl.SEED0 + 5, zhi=1)
+
+
+def test_config5_blocks_small(nk):
+    """prisms + tets, deformed, P=5, lambda=10, ONE nk_helmholtz_apply_blocks call."""
+    n, P, lam = 4, 5, 10.0
+    blocks, refs = [], []
+    for shape, zlo, zhi in ((o.TET, 0, 1), (o.PRISM, 1, 4)):
+        el = K.element(shape, P)
+        A, J = K.geometry(shape, P, n, True, zlo=zlo, zhi=zhi)
+        basis = nk.Basis(shape, P)
+        geom = nk.Geom(basis, A.cuda(), J.cuda(), True)
+        x = wl.coefficients(wl.SEED0 + 5 + shape, J.shape[0], el.Nm)
+        y = torch.full_like(x, float("nan")).cuda()
+        blocks.append((basis, geom, x.cuda(), y))
+        refs.append(o.helmholtz(el, A.numpy(), J.numpy(), lam, x.numpy()))
+    nk.helmholtz_apply_blocks(blocks, lam)
+    torch.cuda.synchronize()
+    for (b, g, x, y), ref in zip(blocks, refs):
+        assert K.normwise_err(y.cpu().numpy(), ref) <= TOL
+
+
+def test_edge_cases(nk):
+    basis = nk.Basis(o.HEX, 2)
+    el = K.element(o.HEX, 2)
+    # nelem = 0: valid, no-op
+    A0 = torch.zeros((0, 1, 3, 3), dtype=torch.float64, device="cuda")
+    J0 = torch.zeros((0, 1), dtype=torch.float64, device="cuda")
+    g0 = nk.Geom(basis, A0, J0, False)
+    x0 = torch.zeros((0, el.Nm), dtype=torch.float64, device="cuda")
+    nk.helmholtz_apply(basis, g0, 1.0, x0, torch.zeros_like(x0) + 1)
+    # nelem = 1 and host-side geometry upload
+    A, J = K.geometry(o.HEX, 2, 2, True, take=torch.tensor([5]))
+    g1 = nk.Geom(basis, A, J, True)            # host tensors
+    x = wl.coefficients(3, 1, el.Nm)
+    y = torch.empty_like(x).cuda()
+    nk.helmholtz_apply(basis, g1, 2.0, x.cuda(), y)
+    ref = o.helmholtz(el, A.numpy(), J.numpy(), 2.0, x.numpy())
+    assert K.normwise_err(y.cpu().numpy(), ref) <= TOL
+    # NULL components of physderiv / iprod_deriv
+    u = wl.point_values(4, 1, el.Nq)
+    d1 = torch.empty_like(u).cuda()
+    nk.physderiv(basis, g1, u.cuda(), None, d1, None)
+    ref = o.physderiv(el, A.numpy(), u.numpy())
+    assert K.normwise_err(d1.cpu().numpy(), ref[1]) <= TOL
+    c = torch.empty((1, el.Nm), dtype=torch.float64, device="cuda")
+    nk.iprod_deriv(basis, g1, None, u.cuda(), None, c)
+    gg = np.stack([np.zeros_like(u.numpy()), u.numpy(), np.zeros_like(u.numpy())])
+    ref = o.iprod_deriv(el, A.numpy(), J.numpy(), gg)
+    assert K.normwise_err(c.cpu().numpy(), ref) <= TOL
+    # errors: aliasing, geometry of another basis
+    with pytest.raises(nk.NkError) as ei:
+        xx = x.cuda()
+        nk.helmholtz_apply(basis, g1, 1.0, xx, xx)
+    assert ei.value.code == 1
+    other = nk.Basis(o.HEX, 3)
+    with pytest.raises(nk.NkError) as ei:
+        nk.helmholtz_apply(other, g1, 1.0, x.cuda(), y)
+    assert ei.value.code == 3
+
+
+def test_operator_identities_on_gpu(nk):
+    """mass = iprod o bwdtrans; laplacian = iprod_deriv o physderiv o bwdtrans;
+    helmholtz = laplacian + lambda mass (SURVEY 8(c) 'Operator identities')."""
+    for shape in (o.HEX, o.TET, o.PRISM):
+        P, lam = 3, 3.5
+        el = K.element(shape, P)
+        A, J = K.geometry(shape, P, 2, True, zhi=1)
+        ne = J.shape[0]
+        basis = nk.Basis(shape, P)
+        geom = nk.Geom(basis, A.cuda(), J.cuda(), True)
+        x = wl.coefficients(11, ne, el.Nm).numpy()
+        u = K.gpu_op(nk, "bwdtrans", basis, geom, lam, x)
+        m1 = K.gpu_op(nk, "iprod", basis, geom, lam, u)
+        m2 = K.gpu_op(nk, "mass", basis, geom, lam, x)
+        assert K.normwise_err(m1, m2) <= 1e-13
+        gr = K.gpu_op(nk, "physderiv", basis, geom, lam, u)
+        l1 = K.gpu_op(nk, "iprod_deriv", basis, geom, lam, gr)
+        l2 = K.gpu_op(nk, "laplacian", basis, geom, lam, x)
+        assert K.normwise_err(l1, l2) <= 1e-13
+        h = K.gpu_op(nk, "helmholtz", basis, geom, lam, x)
+        assert K.normwise_err(h, l2 + lam * m2) <= 1e-13
+
+
+def test_helmholtz_host_entry(nk):
+    P = 4
+    el = K.element(o.HEX, P)
+    A, J = K.geometry(o.HEX, P, 3, True)
+    basis = nk.Basis(o.HEX, P)
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), True)
+    x = wl.coefficients(21, J.shape[0], el.Nm).pin_memory()
+    y = torch.empty_like(x).pin_memory()
+    n0 = nk.launch_count()
+    nk.helmholtz_apply_host(basis, geom, 1.0, x, y)
+    assert nk.launch_count() == n0 + 1
+    ref = o.helmholtz(el, A.numpy(), J.numpy(), 1.0, x.numpy())
+    assert K.normwise_err(y.numpy(), ref) <= TOL
