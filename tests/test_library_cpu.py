@@ -1,0 +1,95 @@
+"""CPU-side checks of libnk (no GPU): the library loads and exports every symbol include/nk.h declares;
+its host tables (closed-form weights, barycentric D, Newton nodes) agree with the oracle's tables, which
+are built from different formulas; mode map; error codes; no CPU fallback."""
+import os
+import re
+
+import numpy as np
+import pytest
+import torch
+
+import golden_io as G
+from oracle import nk_oracle as o
+
+nk = pytest.importorskip("paper_2606_20917_b200.binding", reason="libnk.so not built")
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "nk.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(nk_[a-z0-9_]+)\s*\(", hdr))
+    assert len(declared) >= 24
+    for name in declared:
+        assert hasattr(nk.lib, name), "libnk.so does not export %s" % name
+    assert declared == set(nk.DECLARED_SYMBOLS), declared ^ set(nk.DECLARED_SYMBOLS)
+
+
+@pytest.mark.parametrize("shape", [o.HEX, o.TET, o.PRISM])
+@pytest.mark.parametrize("P", [1, 2, 3, 4, 5, 8])
+def test_host_tables_match_oracle(shape, P):
+    Q = P + 2
+    b = nk.Basis(shape, P)
+    el = o.Element(shape, P, Q)
+    assert (b.num_modes, b.num_points) == (el.Nm, el.Nq)
+    for d in range(3):
+        np.testing.assert_allclose(b.table(nk.TAB_NODES, d).numpy(), el.z[d], atol=2e-15)
+        np.testing.assert_allclose(b.table(nk.TAB_WEIGHTS, d).numpy(), el.w[d], atol=1e-14)
+        D = b.table(nk.TAB_DERIV, d).numpy().reshape(Q, Q)
+        assert np.abs(D - el.D[d]).max() <= 1e-14 * np.abs(el.D[d]).max() * Q
+    np.testing.assert_allclose(b.points().numpy(), el.xi, atol=1e-15)
+    # basis tables against the oracle's 1-D functions
+    nm = P + 1
+    pa = b.table(nk.TAB_PSI, 0).numpy().reshape(Q, nm)
+    for p in range(nm):
+        np.testing.assert_allclose(pa[:, p], o.psi_a(p, el.z[0]), atol=1e-14)
+    if shape != o.HEX:
+        pb = b.table(nk.TAB_PSI, 2).numpy().reshape(Q, nm * (nm + 1) // 2)
+        col = 0
+        for s in range(nm):
+            for r in range(nm - s):
+                np.testing.assert_allclose(pb[:, col], o.psi_b(s, r, el.z[2]), atol=1e-14)
+                col += 1
+    for m, (p, q, r) in enumerate(el.modes):
+        assert b.mode_index(p, q, r) == m
+    assert b.mode_index(P + 1, 0, 0) == -1
+
+
+def test_tet_mode_map_golden():
+    b = nk.Basis(o.TET, 4)
+    for _nm, p, q, r, m in G.records("tet_mode_map.txt"):
+        assert b.mode_index(int(p), int(q), int(r)) == int(m)
+
+
+def test_textbook_quadrature_from_library():
+    b = nk.Basis(o.HEX, 3)           # Q = 5 GLL
+    z = b.table(nk.TAB_NODES, 0).numpy()
+    w = b.table(nk.TAB_WEIGHTS, 0).numpy()
+    np.testing.assert_allclose(z, [-1, -np.sqrt(3 / 7), 0, np.sqrt(3 / 7), 1], atol=1e-15)
+    np.testing.assert_allclose(w, [0.1, 49 / 90, 32 / 45, 49 / 90, 0.1], atol=1e-15)
+    for shape, vol in ((o.HEX, 8.0), (o.TET, 4.0 / 3.0), (o.PRISM, 4.0)):
+        bb = nk.Basis(shape, 4)
+        ws = [bb.table(nk.TAB_WEIGHTS, d).numpy().sum() for d in range(3)]
+        assert np.prod(ws) == pytest.approx(vol, rel=1e-14)      # A16: standard-element volume
+
+
+def test_error_codes_and_no_cpu_fallback():
+    with pytest.raises(nk.NkError) as ei:
+        nk.Basis(o.HEX, 11)
+    assert ei.value.code == 2
+    with pytest.raises(nk.NkError) as ei:
+        nk.Basis(o.TET, 4, Q=7)
+    assert ei.value.code == 2
+    with pytest.raises(nk.NkError) as ei:
+        nk.Basis(7, 4)
+    assert ei.value.code == 1
+    if not torch.cuda.is_available():
+        # compute entry points must refuse to run without a device (no CPU path)
+        import ctypes as C
+        b = nk.Basis(o.HEX, 2)
+        x = torch.zeros(2, b.num_modes, dtype=torch.float64)
+        y = torch.zeros(2, b.num_points, dtype=torch.float64)
+        code = nk.lib.nk_bwdtrans(b.h, 2, x.data_ptr(), y.data_ptr(), None)
+        assert code == 5, nk.lib.nk_last_error()
+        with pytest.raises(ValueError):
+            nk.bwdtrans(b, x, y)

@@ -1,0 +1,63 @@
+"""The five BASELINE.json configurations as seeded synthetic blocks (DATA ONLY, no method
+arithmetic).  A block = dict(shape, P, lam, deformed, v0, E, seed): an affine sub-map per element
+(v0, E) optionally composed with the sinusoidal map of config 2; geometric factors are produced by
+workloads.synthetic from the quadrature-point coordinates `xi` that the caller supplies.
+Recipe and citations: DESIGN.md section 6."""
+import torch
+
+from . import synthetic as wl
+
+HEX, TET, PRISM = 0, 1, 2
+
+
+def _slab(mesh_fn, n, zlo, zhi, device):
+    return mesh_fn(n, zlo, zhi, device=device)
+
+
+def config_blocks(cfg, device="cpu", P_sweep=4, scale=1.0):
+    """Returns (name, op, blocks).  `scale` < 1 shrinks the mesh (tests); 1.0 = BASELINE sizes."""
+    seed = wl.SEED0 + cfg
+    if cfg == 1:
+        v0, E = wl.hex_mesh(4, device=device)
+        return "cfg1 hex affine P3 Q5, 64 el", "helmholtz", [dict(shape=HEX, P=3, lam=1.0, deformed=False, v0=v0, E=E, seed=seed)]
+    if cfg == 2:
+        n = max(2, int(round(32 * scale)))
+        v0, E = wl.hex_mesh(n, device=device)
+        return ("cfg2 hex deformed P4 Q6, %d^3 el" % n, "helmholtz",
+                [dict(shape=HEX, P=4, lam=1.0, deformed=True, v0=v0, E=E, seed=seed)])
+    if cfg == 3:
+        n = max(2, int(round(32 * scale)))
+        v0, E = wl.kuhn_tet_mesh(n, device=device)
+        return ("cfg3 tet affine P4 Q6, 6x%d^3 el" % n, "helmholtz",
+                [dict(shape=TET, P=4, lam=1.0, deformed=False, v0=v0, E=E, seed=seed)])
+    if cfg == 4:
+        n = max(2, int(round(wl.p_sweep_cubes(P_sweep) * scale)))
+        v0, E = wl.hex_mesh(n, device=device)
+        return ("cfg4 hex affine P%d Q%d, %d^3 el" % (P_sweep, P_sweep + 2, n), "mass+laplacian",
+                [dict(shape=HEX, P=P_sweep, lam=0.0, deformed=False, v0=v0, E=E, seed=seed)])
+    if cfg == 5:
+        n = max(4, int(round(40 * scale)))
+        zt = max(1, n // 4)                       # z-layers 0..n/4-1 -> tets, the rest -> prisms
+        vt, Et = wl.kuhn_tet_mesh(n, 0, zt, device=device)
+        vp, Ep = wl.prism_mesh(n, zt, n, device=device)
+        return ("cfg5 hybrid deformed P5 Q7, %d tets + %d prisms" % (vt.shape[0], vp.shape[0]), "helmholtz",
+                [dict(shape=PRISM, P=5, lam=10.0, deformed=True, v0=vp, E=Ep, seed=seed),
+                 dict(shape=TET, P=5, lam=10.0, deformed=True, v0=vt, E=Et, seed=seed + 100)])
+    raise ValueError("config 1..5")
+
+
+def block_factors(block, xi, chunk=4096):
+    """(dxi_dx, detJ) of a block on the device of its mesh; xi [Nq][3] from the caller."""
+    if block["deformed"]:
+        return wl.sinusoidal_factors(block["v0"], block["E"], xi.to(block["v0"].device), chunk=chunk)
+    return wl.affine_factors(block["v0"], block["E"])
+
+
+def shard(block, rank, world):
+    """Contiguous element range of `block` for `rank` (elements are independent: P:163)."""
+    ne = block["v0"].shape[0]
+    lo, hi = ne * rank // world, ne * (rank + 1) // world
+    out = dict(block)
+    out["v0"], out["E"] = block["v0"][lo:hi].contiguous(), block["E"][lo:hi].contiguous()
+    out["range"] = (lo, hi)
+    return out
