@@ -9,7 +9,7 @@ import os
 import torch
 
 HERE = os.path.dirname(os.path.abspath(__file__))
-LIB_PATH = os.path.join(HERE, "libnk.so")
+LIB_PATH = os.environ.get("NK_LIB") or os.path.join(HERE, "libnk.so")   # NK_LIB: another build of the same library
 HEX, TET, PRISM = 0, 1, 2
 TAB_NODES, TAB_WEIGHTS, TAB_DERIV, TAB_PSI = 0, 1, 2, 3
 

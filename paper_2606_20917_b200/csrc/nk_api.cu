@@ -106,16 +106,20 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     b->inst = get();
     const nk::HostTables& t = b->t;
     const int nm = t.nm;
-    // DenseTabs: Ba[Q*nm], D[3][Q*Q], w[3][Q], aux[4][Q]
+    // DenseTabs: Ba[Q*nm], BaT[nm*Q], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
     std::vector<double>& f = b->tabs_flat;
     f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
+    for (int p = 0; p < nm; ++p)
+        for (int i = 0; i < Q; ++i) f.push_back(t.psi[0][i * nm + p]); // BaT
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.D[d].begin(), t.D[d].end());
+    for (int d = 0; d < 3; ++d)
+        for (int r = 0; r < Q; ++r)
+            for (int i = 0; i < Q; ++i) f.push_back(t.D[d][i * Q + r]); // DT
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.w[d].begin(), t.w[d].end());
     for (int i = 0; i < Q; ++i) f.push_back(1.0 + t.z[0][i]);
     for (int i = 0; i < Q; ++i) f.push_back(1.0 + t.z[1][i]);
     for (int i = 0; i < Q; ++i) f.push_back(shape == NK_TET ? 1.0 / (1.0 - t.z[1][i]) : 0.0);
     for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? 1.0 / (1.0 - t.z[2][i]) : 0.0);
-    (void)nm;
     // sparse blob
     nk::SparseOff& so = b->so;
     std::memset(&so, 0, sizeof so);

@@ -24,6 +24,8 @@ static cudaError_t launch(const double* tabs_flat, const SparseOff& so, const KA
     if (blocks_per_sm == 0) {
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
+        err = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
+        if (err != cudaSuccess) return err;
         int bps = 0;
         err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, T::NT, smem);
         if (err != cudaSuccess) return err;

@@ -34,6 +34,13 @@ __device__ __forceinline__ void chain_adj(double c1, double c2, double c3, doubl
     }
 }
 
+// DRAM -> L2 prefetch of a contiguous range (cp.async.bulk.prefetch.L2): one instruction, no
+// registers or shared memory held while the data is in flight.  p 16-byte aligned, bytes % 16 == 0.
+__device__ __forceinline__ void l2_prefetch(const void* p, unsigned bytes)
+{
+    asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 template <int SHAPE, int P, int DEF, int OP>
 __global__ void __launch_bounds__(Tune<SHAPE, P>::NT, Tune<SHAPE, P>::MINB)
 nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_constant__ SparseOff so,
@@ -70,21 +77,32 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
     const double* tab3 = sd + so.tab3;
     const double* tab2 = sd + so.tab2;
 
+#ifdef NK_NO_PERSIST
+    { const int g = blockIdx.x;
+#else
     for (int g = blockIdx.x; g < a.ngroups; g += gridDim.x) {
+#endif
         const long long elem = (long long)g * E + e;
         const bool valid = elem < a.nelem;
         const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
         (void)geo;
+        if constexpr (DEF) {
+            // stream the NEXT group's geometry (contiguous [NCG][NQ][E] doubles) from DRAM into L2 while this
+            // group is being computed: the loads of pass C then hit L2 and HBM stays busy during all stages.
+            const int gn = g + gridDim.x;
+            if (gn < a.ngroups && tid < NCG)
+                l2_prefetch(a.geom + ((size_t)gn * NCG + tid) * NQ * E, (unsigned)(NQ * E * sizeof(double)));
+        }
 
         // ================= input side =================
         if constexpr (IN_COEFF) {
             // a1: coefficients -> Y as C[m]
             const double* __restrict__ src = a.in[0] + elem * NMODES;
-            for (int m = slot; m < NMODES; m += LS) Y[m * E + e] = valid ? __ldg(src + m) : 0.0;
+            NK_FOR(m, NMODES) Y[m * E + e] = valid ? __ldg(src + m) : 0.0;
             __syncthreads();
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
             if constexpr (!SP1) {
-                for (int l = slot; l < NM * NM; l += LS) {
+                NK_FOR(l, NM * NM) {
                     double c[NM];
                     NK_UNROLL for (int r = 0; r < NM; ++r) c[r] = Y[(l * NM + r) * E + e];
                     NK_UNROLL for (int k = 0; k < Q; ++k) {
@@ -97,7 +115,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
                 const int* st = si + so.s1f_start;
                 const int* sr = si + so.s1f_src;
                 const int* rw = si + so.s1f_row;
-                for (int l = slot; l < N1; l += LS) {
+                NK_FOR(l, N1) {
                     double acc[Q];
                     NK_UNROLL for (int k = 0; k < Q; ++k) acc[k] = 0.0;
                     const int e1 = st[l + 1];
@@ -112,7 +130,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
             __syncthreads();
             // a2/S2: sum over q:  T1 -> T2[p][j][k] in X
             if constexpr (!SP2) {
-                for (int l = slot; l < NM * Q; l += LS) {
+                NK_FOR(l, NM * Q) {
                     const int p = l / Q, k = l - p * Q;
                     double c[NM];
                     NK_UNROLL for (int q = 0; q < NM; ++q) c[q] = Z[((p * NM + q) * Q + k) * E + e];
@@ -126,7 +144,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
                 const int* st = si + so.s2f_start;
                 const int* sr = si + so.s2f_src;
                 const int* rw = si + so.s2f_row;
-                for (int l = slot; l < NM * Q; l += LS) {
+                NK_FOR(l, NM * Q) {
                     const int p = l / Q, k = l - p * Q;
                     double acc[Q];
                     NK_UNROLL for (int j = 0; j < Q; ++j) acc[j] = 0.0;

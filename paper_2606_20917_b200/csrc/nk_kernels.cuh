@@ -41,7 +41,7 @@ struct Tune {
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = Q <= 4 ? 32 : Q <= 5 ? 16 : Q <= 8 ? 8 : Q <= 10 ? 4 : 2;
+    static constexpr int E = Q <= 4 ? 32 : Q <= 5 ? 16 : Q <= 7 ? 8 : Q <= 11 ? 4 : 2;
 #endif
     static constexpr int LQ = (E >= 16) ? Q : (Q | 1);
     static constexpr int NQP = LQ * Q * Q;
@@ -49,9 +49,9 @@ struct Tune {
     static constexpr int LS = NK_TUNE_LS;
 #else
     static constexpr int LS_full = Q * Q;
-    // aim at 128..320 threads
-    static constexpr int LS = (E * LS_full <= 320) ? LS_full : (E * ((LS_full + 1) / 2) <= 320) ? (LS_full + 1) / 2
-                              : (E * ((LS_full + 2) / 3) <= 320) ? (LS_full + 2) / 3 : (LS_full + 3) / 4;
+    // one line per thread per pass whenever the block stays within 512 threads: single-trip stages are
+    // straight-line code whose matrix operands are used once (nothing for the compiler to hoist and spill)
+    static constexpr int LS = (E * LS_full <= 512) ? LS_full : (LS_full + 1) / 2;
 #endif
     static constexpr int NT = E * LS;
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
@@ -68,7 +68,11 @@ struct Tune {
 template <int NM, int Q>
 struct DenseTabs {
     double Ba[Q * NM];   // [i][p]  psi^a_p at the GLL points (directions whose basis is psi^a)
+    double BaT[NM * Q];  // [p][i]  the same, transposed: operand of the adjoint passes (Eq. 20).  A second
+                         //         copy at another address also keeps the compiler from holding Ba/D live
+                         //         (and spilling them) between a forward pass and its adjoint.
     double D[3][Q * Q];  // [d][i][r]  D^(d)[i][r] = h_r'(z_i)   (Eq. 22)
+    double DT[3][Q * Q]; // [d][r][i]  transposes
     double w[3][Q];      // 1-D weights (collapse Jacobian folded in, A16)
     double aux[4][Q];    // chain helpers (A17): 1+z1, 1+z2, 1/(1-z2), 1/(1-z3)
 };
@@ -94,5 +98,9 @@ struct KArgs {
 };
 
 #define NK_UNROLL _Pragma("unroll")
+// line loop of a stage: thread `slot` takes lines slot, slot+LS, ...  The trip count is a compile-time
+// constant so that single-trip stages are straight-line code.
+#define NK_FOR(l, N) \
+    _Pragma("unroll 1") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (l < (N))
 
 } // namespace nk
