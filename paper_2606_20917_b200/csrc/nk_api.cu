@@ -106,11 +106,12 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     b->inst = get();
     const nk::HostTables& t = b->t;
     const int nm = t.nm;
-    // DenseTabs: Ba[Q*nm], BaT[nm*Q], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
+    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
     std::vector<double>& f = b->tabs_flat;
-    f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
-    for (int p = 0; p < nm; ++p)
-        for (int i = 0; i < Q; ++i) f.push_back(t.psi[0][i * nm + p]); // BaT
+    for (int d = 0; d < 3; ++d) f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
+    for (int d = 0; d < 3; ++d)
+        for (int p = 0; p < nm; ++p)
+            for (int i = 0; i < Q; ++i) f.push_back(t.psi[0][i * nm + p]); // BaT
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.D[d].begin(), t.D[d].end());
     for (int d = 0; d < 3; ++d)
         for (int r = 0; r < Q; ++r)

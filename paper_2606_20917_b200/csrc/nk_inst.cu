@@ -32,9 +32,9 @@ static cudaError_t launch(const double* tabs_flat, const SparseOff& so, const KA
         blocks_per_sm = bps < 1 ? 1 : bps;
     }
     if (a.ngroups <= 0) return cudaSuccess;
-    const long long cap = (long long)num_sms * blocks_per_sm;
-    const int grid = (int)(a.ngroups < cap ? a.ngroups : cap);
-    kern<<<grid, T::NT, smem, stream>>>(tabs, so, a);
+    KArgs b = a;
+    b.pf_dist = num_sms * blocks_per_sm;
+    kern<<<a.ngroups, T::NT, smem, stream>>>(tabs, so, b);
     return cudaGetLastError();
 }
 

@@ -41,6 +41,14 @@ __device__ __forceinline__ void l2_prefetch(const void* p, unsigned bytes)
     asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
 }
 
+// 8-byte asynchronous global -> shared copy; ok == false writes 0.0 instead (src-size 0)
+__device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, bool ok)
+{
+    const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(ok ? 8 : 0) : "memory");
+}
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
 template <int SHAPE, int P, int DEF, int OP>
 __global__ void __launch_bounds__(Tune<SHAPE, P>::NT, Tune<SHAPE, P>::MINB)
 nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_constant__ SparseOff so,
@@ -77,11 +85,11 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
     const double* tab3 = sd + so.tab3;
     const double* tab2 = sd + so.tab2;
 
-#ifdef NK_NO_PERSIST
-    { const int g = blockIdx.x;
-#else
-    for (int g = blockIdx.x; g < a.ngroups; g += gridDim.x) {
-#endif
+    // one group per block (grid = ngroups).  NOT a persistent loop: ptxas hoists the constant-bank matrix
+    // loads of every stage out of such a loop, holds them in registers and spills them (measured: 300 B of
+    // spills per thread and a third of the issue slots lost).
+    {
+        const int g = blockIdx.x;
         const long long elem = (long long)g * E + e;
         const bool valid = elem < a.nelem;
         const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
@@ -89,16 +97,32 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
         if constexpr (DEF) {
             // stream the NEXT group's geometry (contiguous [NCG][NQ][E] doubles) from DRAM into L2 while this
             // group is being computed: the loads of pass C then hit L2 and HBM stays busy during all stages.
-            const int gn = g + gridDim.x;
+            const int gn = g + a.pf_dist;
             if (gn < a.ngroups && tid < NCG)
                 l2_prefetch(a.geom + ((size_t)gn * NCG + tid) * NQ * E, (unsigned)(NQ * E * sizeof(double)));
         }
 
+        {
+            // the same for the next group's input fields (element-major, contiguous per group)
+            constexpr int NIN = IN_COEFF ? NMODES : NQ;
+            const int gn = g + a.pf_dist;
+            if (gn < a.ngroups && tid == 32) {
+                const double* base = a.in[0];
+                if (base && (reinterpret_cast<size_t>(base) & 15) == 0) {
+                    const long long e0 = (long long)gn * E;
+                    const long long cnt = (a.nelem - e0 < E) ? (a.nelem - e0) : E;
+                    const unsigned bytes = (unsigned)(cnt * NIN * sizeof(double)) & ~15u;
+                    if (bytes) l2_prefetch(base + e0 * NIN, bytes);
+                }
+            }
+        }
         // ================= input side =================
         if constexpr (IN_COEFF) {
             // a1: coefficients -> Y as C[m]
             const double* __restrict__ src = a.in[0] + elem * NMODES;
-            NK_FOR(m, NMODES) Y[m * E + e] = valid ? __ldg(src + m) : 0.0;
+            // LDGSTS (cp.async): every trip in flight at once, no registers held, zero-fill for the ragged tail
+            NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : a.in[0], valid);
+            cp_async_wait_all();
             __syncthreads();
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
             if constexpr (!SP1) {
@@ -107,7 +131,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
                     NK_UNROLL for (int r = 0; r < NM; ++r) c[r] = Y[(l * NM + r) * E + e];
                     NK_UNROLL for (int k = 0; k < Q; ++k) {
                         double acc = 0.0;
-                        NK_UNROLL for (int r = 0; r < NM; ++r) acc = fma(tabs.Ba[k * NM + r], c[r], acc);
+                        NK_UNROLL for (int r = 0; r < NM; ++r) acc = fma(tabs.Ba[2][k * NM + r], c[r], acc);
                         Z[(l * Q + k) * E + e] = acc;
                     }
                 }
@@ -136,7 +160,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
                     NK_UNROLL for (int q = 0; q < NM; ++q) c[q] = Z[((p * NM + q) * Q + k) * E + e];
                     NK_UNROLL for (int j = 0; j < Q; ++j) {
                         double acc = 0.0;
-                        NK_UNROLL for (int q = 0; q < NM; ++q) acc = fma(tabs.Ba[j * NM + q], c[q], acc);
+                        NK_UNROLL for (int q = 0; q < NM; ++q) acc = fma(tabs.Ba[1][j * NM + q], c[q], acc);
                         X[((p * Q + j) * Q + k) * E + e] = acc;
                     }
                 }

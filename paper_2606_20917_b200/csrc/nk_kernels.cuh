@@ -67,10 +67,10 @@ struct Tune {
 // ---- kernel parameters (constant bank) -------------------------------------------------
 template <int NM, int Q>
 struct DenseTabs {
-    double Ba[Q * NM];   // [i][p]  psi^a_p at the GLL points (directions whose basis is psi^a)
-    double BaT[NM * Q];  // [p][i]  the same, transposed: operand of the adjoint passes (Eq. 20).  A second
-                         //         copy at another address also keeps the compiler from holding Ba/D live
-                         //         (and spilling them) between a forward pass and its adjoint.
+    double Ba[3][Q * NM];  // [d][i][p]  psi^a_p at the GLL points, one copy per direction that uses it
+    double BaT[3][NM * Q]; // [d][p][i]  transposes: operands of the adjoint passes (Eq. 20).
+                           // One copy per use site on purpose: loads of one address would be merged by the
+                           // compiler, kept in registers from a forward pass to its adjoint, and spilled.
     double D[3][Q * Q];  // [d][i][r]  D^(d)[i][r] = h_r'(z_i)   (Eq. 22)
     double DT[3][Q * Q]; // [d][r][i]  transposes
     double w[3][Q];      // 1-D weights (collapse Jacobian folded in, A16)
@@ -95,11 +95,15 @@ struct KArgs {
     double lambda;
     long long nelem;
     int ngroups;
+    int pf_dist;             // L2 prefetch distance in groups = number of co-resident blocks
 };
 
 #define NK_UNROLL _Pragma("unroll")
 // line loop of a stage: thread `slot` takes lines slot, slot+LS, ...  The trip count is a compile-time
 // constant so that single-trip stages are straight-line code.
+// NK_FORU: the same, fully unrolled (global loads/stores: all trips in flight at once)
+#define NK_FORU(l, N) \
+    _Pragma("unroll") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (l < (N))
 #define NK_FOR(l, N) \
     _Pragma("unroll 1") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (l < (N))
 
