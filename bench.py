@@ -248,10 +248,12 @@ def main():
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     n0 = nk.launch_count()
     barrier()
+    torch.cuda.nvtx.range_push("nk_timed")     # lets `ncu --nvtx --nvtx-include "nk_timed/"` list exactly these launches
     e0.record()
     for i in range(args.steps):
         step(i)
     e1.record()
+    torch.cuda.nvtx.range_pop()
     barrier()
     launches = nk.launch_count() - n0
     ms = e0.elapsed_time(e1)
