@@ -1,0 +1,101 @@
+"""GPU parity at BASELINE.json's FULL sizes (configs 2, 3 and 5), in the launch configuration that
+bench.py times (same generators, same calls), on sampled elements that the oracle computes one by one.
+The sample always holds the first and last element, both ends of an interleave group, the ragged tail
+of the last group and seeded random elements.  Gate: normwise 1e-12 (A18)."""
+import numpy as np
+import pytest
+import torch
+
+import nk_cases as K
+from oracle import nk_oracle as o
+from workloads import configs as cfgs
+from workloads import synthetic as wl
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-12
+
+
+@pytest.fixture(scope="module")
+def nk():
+    import paper_2606_20917_b200 as nk
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    return nk
+
+
+def sample_elements(ne, E, seed, nrand=48):
+    fixed = [0, 1, E - 1, E, 2 * E - 1, ne // 2, ne - E - 1, ne - E, ne - 2, ne - 1]
+    rng = np.random.Generator(np.random.Philox(seed))
+    idx = sorted(set(int(i) for i in fixed if 0 <= i < ne) | set(int(i) for i in rng.integers(0, ne, nrand)))
+    return torch.tensor(idx, dtype=torch.long)
+
+
+def run_full(nk, cfg):
+    dev = torch.device("cuda", 0)
+    title, op, blocks = cfgs.config_blocks(cfg, device=dev)
+    assert op == "helmholtz"
+    work = []
+    for b in blocks:
+        basis = nk.Basis(b["shape"], b["P"])
+        A, J = cfgs.block_factors(b, basis.points())
+        geom = nk.Geom(basis, A, J, b["deformed"])
+        ne = J.shape[0]
+        x = wl.coefficients(b["seed"], ne, basis.num_modes).to(dev)
+        y = torch.full_like(x, float("nan"))
+        idx = sample_elements(ne, basis.interleave, b["seed"])
+        As, Js = A[idx.to(dev)].cpu(), J[idx.to(dev)].cpu()
+        del A, J
+        work.append((b, basis, geom, x, y, idx, As, Js))
+    lam = blocks[0]["lam"]
+    if len(work) == 1:
+        b, basis, geom, x, y = work[0][:5]
+        nk.helmholtz_apply(basis, geom, lam, x, y)
+    else:
+        nk.helmholtz_apply_blocks([(w[1], w[2], w[3], w[4]) for w in work], lam)
+    torch.cuda.synchronize()
+    worst = 0.0
+    for b, basis, geom, x, y, idx, As, Js in work:
+        assert torch.isfinite(y).all(), "non-finite output in %s" % title
+        el = K.element(b["shape"], b["P"])
+        # the oracle evaluates the geometry of the sampled elements at ITS OWN quadrature points
+        v0, E = b["v0"][idx.to(dev)].cpu(), b["E"][idx.to(dev)].cpu()
+        Ao, Jo = (wl.sinusoidal_factors(v0, E, el.xi) if b["deformed"] else wl.affine_factors(v0, E))
+        assert np.abs(Ao.numpy() - As.numpy()).max() <= 1e-9 * np.abs(Ao.numpy()).max()
+        ref = o.helmholtz(el, Ao.numpy(), Jo.numpy(), b["lam"], x[idx.to(dev)].cpu().numpy())
+        err = K.normwise_err(y[idx.to(dev)].cpu().numpy(), ref)
+        worst = max(worst, err)
+        assert err <= TOL, "%s shape %d: normwise error %.3e on %d sampled elements" % (title, b["shape"], err, len(idx))
+    return worst
+
+
+def test_config2_full_size(nk):
+    run_full(nk, 2)
+
+
+def test_config3_full_size(nk):
+    run_full(nk, 3)
+
+
+def test_config5_full_size(nk):
+    run_full(nk, 5)
+
+
+@pytest.mark.parametrize("P", [1, 4, 7, 10])
+def test_config4_full_size_sampled(nk, P):
+    """config 4 (hex affine P-sweep, ~5e7 DoF): mass and Laplacian applied separately, sampled elements."""
+    dev = torch.device("cuda", 0)
+    title, op, blocks = cfgs.config_blocks(4, device=dev, P_sweep=P)
+    b = blocks[0]
+    basis = nk.Basis(b["shape"], P)
+    A, J = cfgs.block_factors(b, basis.points())
+    geom = nk.Geom(basis, A, J, False)
+    ne = J.shape[0]
+    x = wl.coefficients(b["seed"], ne, basis.num_modes).to(dev)
+    ym, yl = torch.full_like(x, float("nan")), torch.full_like(x, float("nan"))
+    nk.mass_apply(basis, geom, x, ym)
+    nk.laplacian_apply(basis, geom, x, yl)
+    torch.cuda.synchronize()
+    idx = sample_elements(ne, basis.interleave, b["seed"], nrand=16 if P > 6 else 48).to(dev)
+    el = K.element(o.HEX, P)
+    An, Jn, xn = A[idx].cpu().numpy(), J[idx].cpu().numpy(), x[idx].cpu().numpy()
+    assert K.normwise_err(ym[idx].cpu().numpy(), o.mass(el, Jn, xn)) <= TOL
+    assert K.normwise_err(yl[idx].cpu().numpy(), o.laplacian(el, An, Jn, xn)) <= TOL
