@@ -69,8 +69,9 @@ nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** out);
 nk_status nk_basis_destroy(nk_basis* b);
 int nk_basis_num_modes(const nk_basis* b);  /* Nm; -1 if b is NULL */
 int nk_basis_num_points(const nk_basis* b); /* Nq = Q^3           */
-int nk_basis_interleave(const nk_basis* b); /* E: elements per thread block = width of the internal
-                                               element-interleaved layout (A12) */
+int nk_basis_interleave(const nk_basis* b, int deformed); /* E: elements per thread block = width of the
+                                               internal element-interleaved layout (A12) of affine (0) or
+                                               deformed (1) blocks */
 /* copies table `which` of direction dir (0,1,2) into host_out; cap = capacity in doubles.
  * NK_ERR_INVALID_ARG if cap is too small.  *count (may be NULL) receives the number of doubles.    */
 nk_status nk_basis_get_table(const nk_basis* b, int which, int dir, double* host_out, size_t cap, size_t* count);

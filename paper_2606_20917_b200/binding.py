@@ -24,7 +24,7 @@ _SIG = {
     "nk_basis_destroy": (_i, [_p]),
     "nk_basis_num_modes": (_i, [_p]),
     "nk_basis_num_points": (_i, [_p]),
-    "nk_basis_interleave": (_i, [_p]),
+    "nk_basis_interleave": (_i, [_p, _i]),
     "nk_basis_get_table": (_i, [_p, _i, _i, C.POINTER(_d), _sz, C.POINTER(_sz)]),
     "nk_basis_mode_index": (_i, [_p, _i, _i, _i]),
     "nk_basis_get_points": (_i, [_p, C.POINTER(_d), _sz]),
@@ -98,7 +98,7 @@ class Basis:
         self.h, self.shape, self.P, self.Q = h, shape, P, Q
         self.num_modes = lib.nk_basis_num_modes(h)
         self.num_points = lib.nk_basis_num_points(h)
-        self.interleave = lib.nk_basis_interleave(h)
+        self.interleave = (lib.nk_basis_interleave(h, 0), lib.nk_basis_interleave(h, 1))   # (affine, deformed)
 
     def table(self, which, direction):
         n = _sz()

@@ -158,7 +158,7 @@ extern "C" nk_status nk_basis_destroy(nk_basis* b)
 
 extern "C" int nk_basis_num_modes(const nk_basis* b) { return b ? b->t.Nm : -1; }
 extern "C" int nk_basis_num_points(const nk_basis* b) { return b ? b->t.Nq : -1; }
-extern "C" int nk_basis_interleave(const nk_basis* b) { return b ? b->inst->E : -1; }
+extern "C" int nk_basis_interleave(const nk_basis* b, int deformed) { return b ? b->inst->E[deformed ? 1 : 0] : -1; }
 
 extern "C" nk_status nk_basis_get_table(const nk_basis* b, int which, int dir, double* host_out, size_t cap, size_t* count)
 {
@@ -304,7 +304,7 @@ extern "C" nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deform
     g->b = b;
     g->nelem = nelem;
     g->deformed = deformed ? 1 : 0;
-    g->E = b->inst->E;
+    g->E = b->inst->E[g->deformed];
     g->ngroups = (nelem + g->E - 1) / g->E;
     *out = g;
     if (nelem == 0) return NK_OK;
@@ -400,7 +400,7 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     if (st != NK_OK) return st;
     st = ensure_sparse_on_device(b);
     if (st != NK_OK) return st;
-    const int E = b->inst->E;
+    const int E = b->inst->E[(g && g->deformed) ? 1 : 0];
     nk::KArgs a;
     a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
     a.out[0] = out0; a.out[1] = out1; a.out[2] = out2;

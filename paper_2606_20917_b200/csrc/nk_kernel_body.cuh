@@ -50,11 +50,11 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, 
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <int SHAPE, int P, int DEF, int OP>
-__global__ void __launch_bounds__(Tune<SHAPE, P>::NT, Tune<SHAPE, P>::MINB)
+__global__ void __launch_bounds__(Tune<SHAPE, P, DEF>::NT, Tune<SHAPE, P, DEF>::MINB)
 nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_constant__ SparseOff so,
           const __grid_constant__ KArgs a)
 {
-    using T = Tune<SHAPE, P>;
+    using T = Tune<SHAPE, P, DEF>;
     constexpr int NM = P + 1, Q = P + 2, E = T::E, LS = T::LS, LQ = T::LQ;
     constexpr int NQ = Q * Q * Q, NQP = T::NQP, NMODES = k_num_modes(SHAPE, NM);
     constexpr bool IN_COEFF = (OP == OP_BWD || OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);

@@ -31,35 +31,39 @@ __host__ __device__ constexpr int k_num_modes(int shape, int nm)
     return shape == K_HEX ? nm * nm * nm : shape == K_TET ? nm * (nm + 1) * (nm + 2) / 6 : nm * nm * (nm + 1) / 2;
 }
 
-// ---- launch configuration per (shape, P); Q = P+2 --------------------------------------
+// ---- launch configuration per (shape, P, deformed); Q = P+2 -----------------------------
 // E  = elements per group (interleave width), LS = line slots, threads = E*LS,
 // LQ = padded length of an i-line in the point arrays (odd when E < 16 so that the
 //      (j,k)-line pass stays bank-conflict-free), MINB = blocks per SM asked of ptxas.
-template <int SHAPE, int P>
+// Values from the round-1 sweeps on B200 (profiles/r1_notes.md): deformed (HBM-bound) kernels want small
+// blocks (about 150-200 threads) at up to 96 registers, many of them per SM; affine (issue / shared-memory
+// bound) kernels want 72 registers and as many resident threads as that allows.
+template <int SHAPE, int P, int DEF>
 struct Tune {
     static constexpr int Q = P + 2;
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = Q <= 4 ? 32 : Q <= 5 ? 16 : Q <= 7 ? 8 : Q <= 11 ? 4 : 2;
+    static constexpr int E = DEF ? (Q <= 3 ? 16 : Q <= 5 ? 8 : Q <= 8 ? 4 : 2)
+                                 : (Q <= 3 ? 32 : Q <= 4 ? 16 : Q <= 6 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8 : Q <= 10 ? 4 : 2);
 #endif
     static constexpr int LQ = (E >= 16) ? Q : (Q | 1);
     static constexpr int NQP = LQ * Q * Q;
 #if defined(NK_TUNE_LS)
     static constexpr int LS = NK_TUNE_LS;
 #else
-    static constexpr int LS_full = Q * Q;
-    // one line per thread per pass whenever the block stays within 512 threads: single-trip stages are
-    // straight-line code whose matrix operands are used once (nothing for the compiler to hoist and spill)
-    static constexpr int LS = (E * LS_full <= 512) ? LS_full : (LS_full + 1) / 2;
+    // one line per thread per pass: single-trip stages are straight-line code whose matrix operands are
+    // used once (nothing for the compiler to hoist and spill)
+    static constexpr int LS = Q * Q;
 #endif
     static constexpr int NT = E * LS;
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
+    static constexpr int REGS = DEF ? 96 : 72;
     static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + 2048));
-    static constexpr int MINB_reg = 65536 / (NT * 104);
+    static constexpr int MINB_reg = 65536 / (NT * REGS);
     static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
 #endif
 };

@@ -10,8 +10,9 @@ typedef cudaError_t (*LaunchFn)(const double* tabs_flat, const SparseOff& so, co
                                 cudaStream_t stream);
 
 struct InstInfo {
-    int shape, P, Q, E, threads, blocks_per_sm_hint;
-    size_t smem_grid;
+    int shape, P, Q;
+    int E[2], threads[2], blocks_per_sm_hint[2]; // [deformed]
+    size_t smem_grid[2];
     LaunchFn fn[2][OP_COUNT]; // [deformed][op]
 };
 

@@ -41,7 +41,7 @@ def run_full(nk, cfg):
         ne = J.shape[0]
         x = wl.coefficients(b["seed"], ne, basis.num_modes).to(dev)
         y = torch.full_like(x, float("nan"))
-        idx = sample_elements(ne, basis.interleave, b["seed"])
+        idx = sample_elements(ne, basis.interleave[int(b["deformed"])], b["seed"])
         As, Js = A[idx.to(dev)].cpu(), J[idx.to(dev)].cpu()
         del A, J
         work.append((b, basis, geom, x, y, idx, As, Js))
@@ -94,7 +94,7 @@ def test_config4_full_size_sampled(nk, P):
     nk.mass_apply(basis, geom, x, ym)
     nk.laplacian_apply(basis, geom, x, yl)
     torch.cuda.synchronize()
-    idx = sample_elements(ne, basis.interleave, b["seed"], nrand=16 if P > 6 else 48).to(dev)
+    idx = sample_elements(ne, basis.interleave[0], b["seed"], nrand=16 if P > 6 else 48).to(dev)
     el = K.element(o.HEX, P)
     An, Jn, xn = A[idx].cpu().numpy(), J[idx].cpu().numpy(), x[idx].cpu().numpy()
     assert K.normwise_err(ym[idx].cpu().numpy(), o.mass(el, Jn, xn)) <= TOL

@@ -14,23 +14,29 @@ def _slab(mesh_fn, n, zlo, zhi, device):
     return mesh_fn(n, zlo, zhi, device=device)
 
 
-def config_blocks(cfg, device="cpu", P_sweep=4, scale=1.0):
+def config_blocks(cfg, device="cpu", P_sweep=None, scale=1.0):
     """Returns (name, op, blocks).  `scale` < 1 shrinks the mesh (tests); 1.0 = BASELINE sizes."""
     seed = wl.SEED0 + cfg
     if cfg == 1:
         v0, E = wl.hex_mesh(4, device=device)
         return "cfg1 hex affine P3 Q5, 64 el", "helmholtz", [dict(shape=HEX, P=3, lam=1.0, deformed=False, v0=v0, E=E, seed=seed)]
     if cfg == 2:
-        n = max(2, int(round(32 * scale)))
+        # P_sweep: the same workload at another order, cube count chosen to keep the DoF of the P=4 case
+        P = 4 if P_sweep is None else P_sweep
+        n0 = 32 if P == 4 else (32 ** 3 * 125.0 / (P + 1) ** 3) ** (1.0 / 3.0)
+        n = max(2, int(round(n0 * scale)))
         v0, E = wl.hex_mesh(n, device=device)
-        return ("cfg2 hex deformed P4 Q6, %d^3 el" % n, "helmholtz",
-                [dict(shape=HEX, P=4, lam=1.0, deformed=True, v0=v0, E=E, seed=seed)])
+        return ("cfg2 hex deformed P%d Q%d, %d^3 el" % (P, P + 2, n), "helmholtz",
+                [dict(shape=HEX, P=P, lam=1.0, deformed=True, v0=v0, E=E, seed=seed)])
     if cfg == 3:
-        n = max(2, int(round(32 * scale)))
+        P = 4 if P_sweep is None else P_sweep
+        n0 = 32 if P == 4 else (32 ** 3 * 35.0 * 6 / ((P + 1) * (P + 2) * (P + 3))) ** (1.0 / 3.0)
+        n = max(2, int(round(n0 * scale)))
         v0, E = wl.kuhn_tet_mesh(n, device=device)
-        return ("cfg3 tet affine P4 Q6, 6x%d^3 el" % n, "helmholtz",
-                [dict(shape=TET, P=4, lam=1.0, deformed=False, v0=v0, E=E, seed=seed)])
+        return ("cfg3 tet affine P%d Q%d, 6x%d^3 el" % (P, P + 2, n), "helmholtz",
+                [dict(shape=TET, P=P, lam=1.0, deformed=False, v0=v0, E=E, seed=seed)])
     if cfg == 4:
+        P_sweep = 4 if P_sweep is None else P_sweep
         n = max(2, int(round(wl.p_sweep_cubes(P_sweep) * scale)))
         v0, E = wl.hex_mesh(n, device=device)
         return ("cfg4 hex affine P%d Q%d, %d^3 el" % (P_sweep, P_sweep + 2, n), "mass+laplacian",
