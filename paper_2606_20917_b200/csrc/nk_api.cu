@@ -67,12 +67,7 @@ struct nk_basis {
     nk::HostTables t;
     const nk::InstInfo* inst = nullptr;
     std::vector<double> tabs_flat; // DenseTabs<nm,Q> in declaration order
-    nk::SparseOff so;
-    std::vector<double> sp_d;
-    std::vector<int> sp_i;
-    mutable double* d_sp_d = nullptr;
-    mutable int* d_sp_i = nullptr;
-    mutable std::mutex mu;
+    std::vector<double> sx_flat;   // SimplexTabs in declaration order (simplices only)
 };
 
 struct nk_geom {
@@ -121,27 +116,15 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     for (int i = 0; i < Q; ++i) f.push_back(1.0 + t.z[1][i]);
     for (int i = 0; i < Q; ++i) f.push_back(shape == NK_TET ? 1.0 / (1.0 - t.z[1][i]) : 0.0);
     for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? 1.0 / (1.0 - t.z[2][i]) : 0.0);
-    // sparse blob
-    nk::SparseOff& so = b->so;
-    std::memset(&so, 0, sizeof so);
+    // SimplexTabs: b3f, b3a (psi^b at the direction-3 points), b2f, b2a (direction 2; tet only)
     if (shape != NK_HEX) {
-        so.tab3 = (int)b->sp_d.size();
-        b->sp_d.insert(b->sp_d.end(), t.tab3.begin(), t.tab3.end());
-        so.tab2 = (int)b->sp_d.size();
-        b->sp_d.insert(b->sp_d.end(), t.tab2.begin(), t.tab2.end());
-        auto put = [&](const std::vector<int>& v) {
-            const int off = (int)b->sp_i.size();
-            b->sp_i.insert(b->sp_i.end(), v.begin(), v.end());
-            return off;
-        };
-        so.s1f_start = put(t.s1f.start); so.s1f_src = put(t.s1f.src); so.s1f_row = put(t.s1f.row);
-        so.s1a_start = put(t.s1a.start); so.s1a_src = put(t.s1a.src); so.s1a_row = put(t.s1a.row);
-        so.s2f_start = put(t.s2f.start); so.s2f_src = put(t.s2f.src); so.s2f_row = put(t.s2f.row);
-        so.s2a_start = put(t.s2a.start); so.s2a_src = put(t.s2a.src); so.s2a_row = put(t.s2a.row);
-        if (b->sp_d.size() % 2) b->sp_d.push_back(0.0);
-        if (b->sp_i.size() % 2) b->sp_i.push_back(0);
-        so.ndoubles = (int)b->sp_d.size();
-        so.nints = (int)b->sp_i.size();
+        std::vector<double>& x = b->sx_flat;
+        const size_t n = (size_t)t.npair * Q;
+        for (int c = 0; c < 2; ++c) x.insert(x.end(), t.tab3.begin(), t.tab3.end());
+        for (int c = 0; c < 2; ++c) {
+            if (shape == NK_TET) x.insert(x.end(), t.tab2.begin(), t.tab2.end());
+            else x.insert(x.end(), n, 0.0);
+        }
     }
     *out = b;
     return NK_OK;
@@ -150,8 +133,6 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
 extern "C" nk_status nk_basis_destroy(nk_basis* b)
 {
     if (!b) return NK_OK;
-    if (b->d_sp_d) cudaFree(b->d_sp_d);
-    if (b->d_sp_i) cudaFree(b->d_sp_i);
     delete b;
     return NK_OK;
 }
@@ -269,25 +250,6 @@ __global__ void repack_kernel(const __grid_constant__ RepackTabs rt, const doubl
     }
 }
 
-nk_status ensure_sparse_on_device(const nk_basis* b)
-{
-    if (b->t.shape == nk::HEX || b->d_sp_d) return NK_OK;
-    std::lock_guard<std::mutex> lk(b->mu);
-    if (b->d_sp_d) return NK_OK;
-    double* dd = nullptr;
-    int* di = nullptr;
-    cudaError_t e = cudaMalloc(&dd, b->sp_d.size() * sizeof(double));
-    if (e != cudaSuccess) return cuda_fail(e, "cudaMalloc(sparse tables)");
-    e = cudaMalloc(&di, b->sp_i.size() * sizeof(int));
-    if (e != cudaSuccess) { cudaFree(dd); return cuda_fail(e, "cudaMalloc(sparse tables)"); }
-    e = cudaMemcpy(dd, b->sp_d.data(), b->sp_d.size() * sizeof(double), cudaMemcpyHostToDevice);
-    if (e == cudaSuccess) e = cudaMemcpy(di, b->sp_i.data(), b->sp_i.size() * sizeof(int), cudaMemcpyHostToDevice);
-    if (e != cudaSuccess) { cudaFree(dd); cudaFree(di); return cuda_fail(e, "cudaMemcpy(sparse tables)"); }
-    b->d_sp_i = di;
-    b->d_sp_d = dd;
-    return NK_OK;
-}
-
 } // namespace
 
 extern "C" nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
@@ -398,8 +360,6 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     if (in0 && (in0 == out0)) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": in and out alias");
     nk_status st = ensure_device();
     if (st != NK_OK) return st;
-    st = ensure_sparse_on_device(b);
-    if (st != NK_OK) return st;
     const int E = b->inst->E[(g && g->deformed) ? 1 : 0];
     nk::KArgs a;
     a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
@@ -410,14 +370,12 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
         def = g->deformed;
         a.geom = (op == nk::OP_PHYSDERIV || op == nk::OP_IPDERIV) ? g->d_factor : g->d_metric;
     }
-    a.sparse_d = b->d_sp_d;
-    a.sparse_i = b->d_sp_i;
     a.lambda = lambda;
     a.nelem = nelem;
     const int64_t ngroups = (nelem + E - 1) / E;
     if (ngroups > 0x7fffffffLL) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": too many elements");
     a.ngroups = (int)ngroups;
-    cudaError_t e = b->inst->fn[def][op](b->tabs_flat.data(), b->so, a, g_num_sms, (cudaStream_t)stream);
+    cudaError_t e = b->inst->fn[def][op](b->tabs_flat.data(), b->sx_flat.data(), a, g_num_sms, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, name);
     { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
     return NK_OK;

@@ -176,25 +176,6 @@ static void bary_deriv(const std::vector<double>& z, std::vector<double>& D)
     }
 }
 
-static void add_entry(std::vector<std::vector<std::pair<int, int>>>& lists, int out, int src, int row)
-{
-    lists[out].push_back({src, row});
-}
-
-static SparseStage flatten(const std::vector<std::vector<std::pair<int, int>>>& lists)
-{
-    SparseStage s;
-    s.start.push_back(0);
-    for (auto& l : lists) {
-        for (auto& e : l) {
-            s.src.push_back(e.first);
-            s.row.push_back(e.second);
-        }
-        s.start.push_back((int)s.src.size());
-    }
-    return s;
-}
-
 bool build_host_tables(int shape, int P, int Q, HostTables& t)
 {
     if (shape < HEX || shape > PRISM || P < 1 || Q < 3) return false;
@@ -252,59 +233,13 @@ bool build_host_tables(int shape, int P, int Q, HostTables& t)
     t.tab3.assign((size_t)t.npair * Q, 0.0);
     for (int row = 0; row < t.npair; ++row)
         for (int k = 0; k < Q; ++k) t.tab3[(size_t)row * Q + k] = t.psi[2][(size_t)k * t.npair + row];
-    const int row01 = pair_index(nm, 0, 1);
-    using Lists = std::vector<std::vector<std::pair<int, int>>>;
     if (shape == TET) {
         t.n1 = t.npair;
         t.tab2.assign((size_t)t.npair * Q, 0.0);
         for (int row = 0; row < t.npair; ++row)
             for (int j = 0; j < Q; ++j) t.tab2[(size_t)row * Q + j] = t.psi[1][(size_t)j * t.npair + row];
-        Lists f1(t.n1), a1(t.Nm), f2(nm), a2(t.n1);
-        for (int p = 0; p < nm; ++p)
-            for (int q = 0; q < nm - p; ++q) {
-                const int l = pair_index(nm, p, q);
-                for (int r = 0; r < nm - p - q; ++r) {
-                    const int m = mode_index(TET, nm, p, q, r), row = pair_index(nm, p + q, r);
-                    add_entry(f1, l, m, row);
-                    add_entry(a1, m, l, row);
-                }
-                add_entry(f2, p, l, l); // tab2 row of (p,q) is the pair index itself
-                add_entry(a2, l, p, l);
-            }
-        // A8: top vertex (0,0,1) also feeds the (0,1) and (1,0) columns after the r-sum;
-        //     the (0,1) column also feeds row p=1 after the q-sum.
-        const int m001 = mode_index(TET, nm, 0, 0, 1);
-        const int l01 = pair_index(nm, 0, 1), l10 = pair_index(nm, 1, 0);
-        add_entry(f1, l01, m001, row01);
-        add_entry(f1, l10, m001, row01);
-        add_entry(a1, m001, l01, row01);
-        add_entry(a1, m001, l10, row01);
-        add_entry(f2, 1, l01, l01);
-        add_entry(a2, l01, 1, l01);
-        t.s1f = flatten(f1);
-        t.s1a = flatten(a1);
-        t.s2f = flatten(f2);
-        t.s2a = flatten(a2);
-    } else { // PRISM: lines (p,q) dense in q, r <= P-p
+    } else {
         t.n1 = nm * nm;
-        Lists f1(t.n1), a1(t.Nm);
-        for (int p = 0; p < nm; ++p)
-            for (int q = 0; q < nm; ++q) {
-                const int l = p * nm + q;
-                for (int r = 0; r < nm - p; ++r) {
-                    const int m = mode_index(PRISM, nm, p, q, r), row = pair_index(nm, p, r);
-                    add_entry(f1, l, m, row);
-                    add_entry(a1, m, l, row);
-                }
-            }
-        // A8: modes (0,q,1) on the collapsed edge also feed row p=1 after the r-sum.
-        for (int q = 0; q < nm; ++q) {
-            const int m = mode_index(PRISM, nm, 0, q, 1), l = 1 * nm + q;
-            add_entry(f1, l, m, row01);
-            add_entry(a1, m, l, row01);
-        }
-        t.s1f = flatten(f1);
-        t.s1a = flatten(a1);
     }
     return true;
 }

@@ -8,25 +8,17 @@ namespace nk {
 
 enum { HEX = 0, TET = 1, PRISM = 2 };
 
-// A sparse "line stage": output o = sum over entries en in [start[o], start[o+1]) of
-// input[src[en]] (x) table row row[en].  These are the index arrays that replace the
-// triangular loop nests of Eq. 17 / Eq. 21 (cf. the index arrays of P:302)
-// and carry the top-vertex / top-edge corrections of A8 as ordinary entries.
-struct SparseStage {
-    std::vector<int> start, src, row;
-};
-
 struct HostTables {
     int shape = 0, P = 0, Q = 0, nm = 0, Nm = 0, Nq = 0, npair = 0;
     std::vector<double> z[3], w[3]; // nodes; weights with the collapse Jacobian folded in (A16)
     std::vector<double> D[3];       // D[d][i*Q + r] = h_r'(z_i)   (Eq. 22)
     int ncol[3] = {0, 0, 0};
     std::vector<double> psi[3];     // psi[d][i*ncol[d] + col]   (point-major, see nk.h NK_TAB_PSI)
-    // simplices only
+    // simplices only: row-major copies of psi[2] / psi[1] (constant-bank operands of the triangular stages,
+    // Eq. 17 / Eq. 21; the A8 corrections are compile-time special cases in csrc/nk_stage_sx.inc)
     int n1 = 0;                     // number of (p,q) lines after the r-sum
     std::vector<double> tab3;       // [row][k]  psi^b_{s,r}(z3_k), row = pair(s,r)
     std::vector<double> tab2;       // [row][j]  psi^b_{p,q}(z2_j), row = pair(p,q)   (tet)
-    SparseStage s1f, s1a, s2f, s2a;
 };
 
 // Jacobi polynomial P_n^{a,b}(x) (A7)

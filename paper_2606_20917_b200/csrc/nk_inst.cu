@@ -13,13 +13,19 @@
 namespace nk {
 
 template <int SHAPE, int P, int DEF, int OP>
-static cudaError_t launch(const double* tabs_flat, const SparseOff& so, const KArgs& a, int num_sms, cudaStream_t stream)
+static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const KArgs& a, int num_sms, cudaStream_t stream)
 {
     using T = Tune<SHAPE, P, DEF>;
     static int blocks_per_sm = 0;
     DenseTabs<P + 1, P + 2> tabs;
     std::memcpy(&tabs, tabs_flat, sizeof(tabs));
-    const size_t smem = T::smem_grid + (SHAPE != K_HEX ? (size_t)so.ndoubles * 8 + (size_t)so.nints * 4 : 0);
+    typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st;
+    if (SHAPE != K_HEX)
+        std::memcpy(&st, sx_flat, sizeof(st));
+    else
+        std::memset(&st, 0, sizeof(st));
+    static_assert(sizeof(tabs) + sizeof(st) + sizeof(KArgs) <= 32000, "kernel parameters exceed the 32 KB limit");
+    const size_t smem = T::smem_grid;
     auto kern = nk_kernel<SHAPE, P, DEF, OP>;
     if (blocks_per_sm == 0) {
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
@@ -34,7 +40,7 @@ static cudaError_t launch(const double* tabs_flat, const SparseOff& so, const KA
     if (a.ngroups <= 0) return cudaSuccess;
     KArgs b = a;
     b.pf_dist = num_sms * blocks_per_sm;
-    kern<<<a.ngroups, T::NT, smem, stream>>>(tabs, so, b);
+    kern<<<a.ngroups, T::NT, smem, stream>>>(tabs, st, b);
     return cudaGetLastError();
 }
 

@@ -51,8 +51,8 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 template <int SHAPE, int P, int DEF, int OP>
 __global__ void __launch_bounds__(Tune<SHAPE, P, DEF>::NT, Tune<SHAPE, P, DEF>::MINB)
-nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_constant__ SparseOff so,
-          const __grid_constant__ KArgs a)
+nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
+          const __grid_constant__ typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st, const __grid_constant__ KArgs a)
 {
     using T = Tune<SHAPE, P, DEF>;
     constexpr int NM = P + 1, Q = P + 2, E = T::E, LS = T::LS, LQ = T::LQ;
@@ -70,20 +70,14 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
     double* __restrict__ X = sm;
     double* __restrict__ Y = sm + (size_t)NQP * E;
     double* __restrict__ Z = sm + (size_t)2 * NQP * E;
-    double* sd = sm + (size_t)3 * NQP * E;
-    int* si = reinterpret_cast<int*>(sd + so.ndoubles);
-
     const int tid = threadIdx.x;
     const int e = tid % E, slot = tid / E;
 #define GIDX(i, j, k) (((i) + LQ * ((j) + Q * (k))) * E + e)
 
-    if constexpr (SP1) { // stage the sparse tables once per block
-        for (int t = tid; t < so.ndoubles; t += T::NT) sd[t] = __ldg(a.sparse_d + t);
-        for (int t = tid; t < so.nints; t += T::NT) si[t] = __ldg(a.sparse_i + t);
-        __syncthreads();
-    }
-    const double* tab3 = sd + so.tab3;
-    const double* tab2 = sd + so.tab2;
+    // simplex stages: warp-uniform roles (see nk_stage_sx.inc)
+    constexpr int SPW = T::SPW;
+    const int warp = tid >> 5, sub = (tid & 31) / E;
+    (void)warp; (void)sub; (void)st;
 
     // one group per block (grid = ngroups).  NOT a persistent loop: ptxas hoists the constant-bank matrix
     // loads of every stage out of such a loop, holds them in registers and spills them (measured: 300 B of
@@ -136,20 +130,9 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
                     }
                 }
             } else {
-                const int* st = si + so.s1f_start;
-                const int* sr = si + so.s1f_src;
-                const int* rw = si + so.s1f_row;
-                NK_FOR(l, N1) {
-                    double acc[Q];
-                    NK_UNROLL for (int k = 0; k < Q; ++k) acc[k] = 0.0;
-                    const int e1 = st[l + 1];
-                    for (int en = st[l]; en < e1; ++en) {
-                        const double c = Y[sr[en] * E + e];
-                        const double* tb = tab3 + rw[en] * Q;
-                        NK_UNROLL for (int k = 0; k < Q; ++k) acc[k] = fma(c, tb[k], acc[k]);
-                    }
-                    NK_UNROLL for (int k = 0; k < Q; ++k) Z[(l * Q + k) * E + e] = acc[k];
-                }
+#define NK_SX_STAGE 1
+#include "nk_stage_sx.inc"
+#undef NK_SX_STAGE
             }
             __syncthreads();
             // a2/S2: sum over q:  T1 -> T2[p][j][k] in X
@@ -165,21 +148,9 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs, const __grid_con
                     }
                 }
             } else {
-                const int* st = si + so.s2f_start;
-                const int* sr = si + so.s2f_src;
-                const int* rw = si + so.s2f_row;
-                NK_FOR(l, NM * Q) {
-                    const int p = l / Q, k = l - p * Q;
-                    double acc[Q];
-                    NK_UNROLL for (int j = 0; j < Q; ++j) acc[j] = 0.0;
-                    const int e1 = st[p + 1];
-                    for (int en = st[p]; en < e1; ++en) {
-                        const double c = Z[(sr[en] * Q + k) * E + e];
-                        const double* tb = tab2 + rw[en] * Q;
-                        NK_UNROLL for (int j = 0; j < Q; ++j) acc[j] = fma(c, tb[j], acc[j]);
-                    }
-                    NK_UNROLL for (int j = 0; j < Q; ++j) X[((p * Q + j) * Q + k) * E + e] = acc[j];
-                }
+#define NK_SX_STAGE 2
+#include "nk_stage_sx.inc"
+#undef NK_SX_STAGE
             }
             __syncthreads();
 #include "nk_stage_s3.inc"

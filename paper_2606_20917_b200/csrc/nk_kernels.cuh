@@ -21,6 +21,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <type_traits>
+
 namespace nk {
 
 enum { K_HEX = 0, K_TET = 1, K_PRISM = 2 };
@@ -49,19 +51,33 @@ struct Tune {
 #endif
     static constexpr int LQ = (E >= 16) ? Q : (Q | 1);
     static constexpr int NQP = LQ * Q * Q;
+    // On simplices the triangular stages give every WARP one (s) or (p) value, so that the psi^b entries are
+    // warp-uniform constant-bank operands; LS is rounded up to what those stages need.
+    static constexpr int NM = P + 1, SPW = 32 / E;          // SPW = line slots per warp
+    static constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
+    static constexpr int warps_s1_tet()
+    {
+        int w = 0;
+        for (int s = 0; s < NM; ++s) w += cdiv(s + 1, SPW);
+        return w;
+    }
+    static constexpr int WARPS_SX = SHAPE == K_HEX ? 0
+                                    : SHAPE == K_TET ? (warps_s1_tet() > NM * cdiv(Q, SPW) ? warps_s1_tet() : NM * cdiv(Q, SPW))
+                                                     : NM * cdiv(NM, SPW);
+    static constexpr int LS_min = SHAPE == K_HEX ? 0 : WARPS_SX * SPW;
 #if defined(NK_TUNE_LS)
-    static constexpr int LS = NK_TUNE_LS;
+    static constexpr int LS = NK_TUNE_LS > LS_min ? NK_TUNE_LS : LS_min;
 #else
     // one line per thread per pass: single-trip stages are straight-line code whose matrix operands are
     // used once (nothing for the compiler to hoist and spill)
-    static constexpr int LS = Q * Q;
+    static constexpr int LS = SHAPE == K_HEX ? Q * Q : cdiv((Q * Q > LS_min ? Q * Q : LS_min), SPW) * SPW;
 #endif
     static constexpr int NT = E * LS;
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
-    static constexpr int REGS = DEF ? 96 : 72;
+    static constexpr int REGS = DEF ? 96 : 64;
     static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + 2048));
     static constexpr int MINB_reg = 65536 / (NT * REGS);
     static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
@@ -81,26 +97,52 @@ struct DenseTabs {
     double aux[4][Q];    // chain helpers (A17): 1+z1, 1+z2, 1/(1-z2), 1/(1-z3)
 };
 
-struct SparseOff {       // offsets into the sparse blob (doubles first, then ints)
-    int ndoubles, nints;
-    int tab3, tab2;                                  // double offsets
-    int s1f_start, s1f_src, s1f_row;                 // int offsets
-    int s1a_start, s1a_src, s1a_row;
-    int s2f_start, s2f_src, s2f_row;
-    int s2a_start, s2a_src, s2a_row;
+// pair index of the psi^b tables: row (a,b), a+b <= P  ->  sum_{c<a}(nm-c) + b
+__host__ __device__ constexpr int k_pair(int nm, int a, int b) { return a * nm - a * (a - 1) / 2 + b; }
+// storage rank of mode (p,q,0) (Eq. 18, A3)
+__host__ __device__ constexpr int k_tet_mode0(int nm, int p, int q)
+{
+    return p * (3 * nm * nm - 3 * nm * p + 6 * nm + p * p - 3 * p + 2) / 6 + q * (nm - p) - q * (q - 1) / 2;
+}
+__host__ __device__ constexpr int k_prism_mode0(int nm, int p, int q)
+{
+    return nm * (p * nm - p * (p - 1) / 2) + q * (nm - p);
+}
+
+// psi^b tables of the collapsed directions (A7), constant-bank operands of the simplex stages.
+// Row = k_pair(a,b), Q entries per row (contiguous in the point index).  Forward and adjoint stages have
+// their own copies (same reason as DenseTabs).  NRQ = npair*Q on simplices, 1 on hexes (unused).
+template <int NRQ>
+struct SimplexTabs {
+    double b3f[NRQ], b3a[NRQ]; // psi^b_{s,r}(eta3_k): tet s = p+q, prism s = p
+    double b2f[NRQ], b2a[NRQ]; // psi^b_{p,q}(eta2_j): tet only
+};
+template <int SHAPE, int NM, int Q>
+struct SimplexTabsFor {
+    using type = SimplexTabs<(SHAPE == K_HEX) ? 1 : (NM * (NM + 1) / 2) * Q>;
 };
 
 struct KArgs {
     const double* in[3];
     double* out[3];
     const double* geom;      // metric stream (7 comps) or factor stream (10 comps), see nk_api.cu
-    const double* sparse_d;  // device copy of the sparse blob
-    const int* sparse_i;
     double lambda;
     long long nelem;
     int ngroups;
     int pf_dist;             // L2 prefetch distance in groups = number of co-resident blocks
 };
+
+// runtime value -> compile-time constant: f(std::integral_constant<int, v>) for v in [0, N)
+template <int N, class F>
+__device__ __forceinline__ void static_switch(int v, F&& f)
+{
+    if constexpr (N > 0) {
+        if (v == N - 1)
+            f(std::integral_constant<int, N - 1>{});
+        else
+            static_switch<N - 1>(v, static_cast<F&&>(f));
+    }
+}
 
 #define NK_UNROLL _Pragma("unroll")
 // line loop of a stage: thread `slot` takes lines slot, slot+LS, ...  The trip count is a compile-time

@@ -5,8 +5,8 @@
 
 namespace nk {
 
-// tabs_flat: the doubles of DenseTabs<P+1,P+2> in declaration order.
-typedef cudaError_t (*LaunchFn)(const double* tabs_flat, const SparseOff& so, const KArgs& a, int num_sms,
+// tabs_flat / sx_flat: the doubles of DenseTabs<P+1,P+2> / SimplexTabs in declaration order.
+typedef cudaError_t (*LaunchFn)(const double* tabs_flat, const double* sx_flat, const KArgs& a, int num_sms,
                                 cudaStream_t stream);
 
 struct InstInfo {
