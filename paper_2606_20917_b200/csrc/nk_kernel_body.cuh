@@ -73,6 +73,10 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     const int tid = threadIdx.x;
     const int e = tid % E, slot = tid / E;
 #define GIDX(i, j, k) (((i) + LQ * ((j) + Q * (k))) * E + e)
+// partial transforms T1[l][k] (after the r-sum) and T2[p][j][k] (after the q-sum): the k-stride LQ is odd
+// when E < 16, so that threads on consecutive lines l or j fall into different banks
+#define T1IDX(l, k) (((l) * LQ + (k)) * E + e)
+#define T2IDX(p, j, k) ((((p) * Q + (j)) * LQ + (k)) * E + e)
 
     // simplex stages: warp-uniform roles (see nk_stage_sx.inc)
     constexpr int SPW = T::SPW;
@@ -126,7 +130,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
                     NK_UNROLL for (int k = 0; k < Q; ++k) {
                         double acc = 0.0;
                         NK_UNROLL for (int r = 0; r < NM; ++r) acc = fma(tabs.Ba[2][k * NM + r], c[r], acc);
-                        Z[(l * Q + k) * E + e] = acc;
+                        Z[T1IDX(l, k)] = acc;
                     }
                 }
             } else {
@@ -140,11 +144,11 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
                 NK_FOR(l, NM * Q) {
                     const int p = l / Q, k = l - p * Q;
                     double c[NM];
-                    NK_UNROLL for (int q = 0; q < NM; ++q) c[q] = Z[((p * NM + q) * Q + k) * E + e];
+                    NK_UNROLL for (int q = 0; q < NM; ++q) c[q] = Z[T1IDX(p * NM + q, k)];
                     NK_UNROLL for (int j = 0; j < Q; ++j) {
                         double acc = 0.0;
                         NK_UNROLL for (int q = 0; q < NM; ++q) acc = fma(tabs.Ba[1][j * NM + q], c[q], acc);
-                        X[((p * Q + j) * Q + k) * E + e] = acc;
+                        X[T2IDX(p, j, k)] = acc;
                     }
                 }
             } else {
@@ -161,6 +165,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
 #include "nk_stage_out.inc"
     }
 #undef GIDX
+#undef T1IDX
+#undef T2IDX
 }
 
 } // namespace nk
