@@ -1,6 +1,7 @@
 // nk_inst.cu -- explicit instantiation of nk_kernel for ONE (shape, P), Q = P+2; compiled once per
 // pair with -DNK_SHAPE=<0|1|2> -DNK_P=<order>.  Compile-time specialisation over (shape, P, Q,
 // deformed, op) replaces the paper's JIT (north_star).
+#include <cstdlib>
 #include <cstring>
 
 #include "nk_kernel_body.cuh"
@@ -39,7 +40,15 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
     }
     if (a.ngroups <= 0) return cudaSuccess;
     KArgs b = a;
-    b.pf_dist = num_sms * blocks_per_sm;
+    // L2 prefetch distance = 1/8 of the co-resident blocks (B200 sweep, profiles/r1_notes.md: flat between 3 %
+    // and 25 %; at 100 % a third of the prefetched lines are evicted before use and re-read from DRAM).
+    // NK_PREFETCH_PCT rescales it (percent of the co-resident blocks; 0 = off).
+    static int pf_pct = -1;
+    if (pf_pct < 0) {
+        const char* ev = std::getenv("NK_PREFETCH_PCT");
+        pf_pct = ev ? std::atoi(ev) : 12;
+    }
+    b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * pf_pct / 100) + 1 : 0x3fffffff;
     kern<<<a.ngroups, T::NT, smem, stream>>>(tabs, st, b);
     return cudaGetLastError();
 }
