@@ -34,6 +34,8 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=400)
     ap.add_argument("--warmup", type=int, default=50)
     ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--fields", type=int, default=1, help="multi-field block (P:199): N fields share one geometry; "
+                    "single-block Helmholtz workloads only (DESIGN.md section 10)")
     ap.add_argument("--impl", default="nk", choices=["nk", "reference"])
     ap.add_argument("--cpu-seconds", type=float, default=12.0, help="budget of the cpu_baseline leg")
     return ap.parse_args()
@@ -213,12 +215,22 @@ def main():
         ys = [torch.empty_like(xs[0]) for _ in range(NSETS)]
         work.append((basis, geom, xs, ys, b["lam"], ne))
         by, fl = algorithmic(b["shape"], b["P"], b["deformed"], "helmholtz")
-        dof += ne * basis.num_modes
-        alg_bytes += by * ne
-        alg_flops += fl * ne
+        nf = args.fields
+        dof += ne * basis.num_modes * nf
+        alg_bytes += (by + 16 * basis.num_modes * (nf - 1)) * ne      # the geometry is shared by the fields
+        alg_flops += fl * ne * nf
         geom_bytes += 56 * ne * (basis.num_points if b["deformed"] else 1)
     torch.cuda.empty_cache()
     lam = blocks[0]["lam"]
+    fxs = fys = None
+    if args.fields > 1:
+        if len(work) != 1 or op != "helmholtz":
+            raise SystemExit("--fields applies to single-block Helmholtz workloads")
+        basis, geom, xs, ys, _, ne = work[0]
+        # two rotating sets of N fields each
+        fxs = [[wl.coefficients(blocks[0]["seed"] + 10 * r + f, ne, basis.num_modes).to(dev) for f in range(args.fields)]
+               for r in range(2)]
+        fys = [[torch.empty_like(fxs[0][0]) for f in range(args.fields)] for r in range(2)]
 
     def step(i):
         s = i % NSETS
@@ -226,6 +238,9 @@ def main():
             for basis, geom, xs, ys, _, _ in work:
                 nk.mass_apply(basis, geom, xs[s], ys[s])
                 nk.laplacian_apply(basis, geom, xs[s], ys[(s + 1) % NSETS])
+        elif len(work) == 1 and args.fields > 1:
+            basis, geom, xs, ys, l, _ = work[0]
+            nk.helmholtz_apply_fields(basis, geom, l, fxs[s % 2], fys[s % 2])
         elif len(work) == 1:
             basis, geom, xs, ys, l, _ = work[0]
             nk.helmholtz_apply(basis, geom, l, xs[s], ys[s])
@@ -265,7 +280,7 @@ def main():
 
     # ---- end to end: HOST buffers through nk_helmholtz_apply_host (H2D + kernel + D2H per step) ----
     e2e = None
-    if op == "helmholtz":
+    if op == "helmholtz" and args.fields == 1:
         hx = [[x.cpu().pin_memory() for x in w[2][:2]] for w in work]
         hy = [[torch.empty_like(h) for h in hs] for hs in hx]
         hy = [[h.pin_memory() for h in hs] for hs in hy]
@@ -333,7 +348,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": "GDoF/s", "n_gpus": world, "steps": args.steps,
             "warmup": max(args.warmup, 3), "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": title, "op": op, "dof_per_gpu": dof, "lambda": lam,
+            "config": {"workload": title + (" x %d fields" % args.fields if args.fields > 1 else ""), "op": op, "dof_per_gpu": dof, "lambda": lam,
                        "l2": "inputs larger than L2: geometry stream %.0f MB per step + %d rotating coefficient "
                              "buffer sets" % (geom_bytes / 1e6, NSETS),
                        "parallelism": "elements sharded, no collective (dp%d)" % world},

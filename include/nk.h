@@ -117,6 +117,14 @@ nk_status nk_laplacian_apply(const nk_basis* b, const nk_geom* g, const double* 
 nk_status nk_helmholtz_apply(const nk_basis* b, const nk_geom* g, double lambda, const double* in,
                              double* out, void* stream);
 
+/* Multi-field block (the `Fields` attribute of a block): the Helmholtz operator applied to nfields
+ * (1..8) coefficient fields that share one geometry, e.g. the d velocity components of the velocity-correction
+ * scheme, in ONE launch: out[f] = (L + lambda M) in[f].  in / out are HOST arrays of nfields DEVICE
+ * pointers, each field [nelem][Nm]; no in[f] may equal any out[h], outputs must be distinct.  The geometry
+ * stream is read from HBM once per group and shared by the fields through L2.                             */
+nk_status nk_helmholtz_apply_fields(const nk_basis* b, const nk_geom* g, double lambda, int nfields,
+                                    const double* const* in, double* const* out, void* stream);
+
 /* several blocks (possibly of different shape / order) in one call, e.g. a hybrid prism + tet mesh   */
 typedef struct {
     const nk_basis* basis;

@@ -6,7 +6,7 @@ kernels of libnk.so.  Names are resolved lazily so that `python -m paper_2606_20
 can run before the library exists; any other use without a built libnk.so raises.
 """
 _EXPORTS = ("lib", "NkError", "Basis", "Geom", "HEX", "TET", "PRISM", "bwdtrans", "iprod", "physderiv",
-            "iprod_deriv", "mass_apply", "laplacian_apply", "helmholtz_apply", "helmholtz_apply_blocks",
+            "iprod_deriv", "mass_apply", "laplacian_apply", "helmholtz_apply", "helmholtz_apply_fields", "helmholtz_apply_blocks",
             "helmholtz_apply_host", "probe_fp64_peak", "launch_count", "version", "LIB_PATH", "DECLARED_SYMBOLS")
 
 

@@ -38,6 +38,7 @@ _SIG = {
     "nk_mass_apply": (_i, [_p, _p, _p, _p, _p]),
     "nk_laplacian_apply": (_i, [_p, _p, _p, _p, _p]),
     "nk_helmholtz_apply": (_i, [_p, _p, _d, _p, _p, _p]),
+    "nk_helmholtz_apply_fields": (_i, [_p, _p, _d, _i, C.POINTER(_p), C.POINTER(_p), _p]),
     "nk_helmholtz_apply_blocks": (_i, [_i, _p, _d, _p]),
     "nk_helmholtz_apply_host": (_i, [_p, _p, _d, _p, _p, _p]),
     "nk_probe_fp64_peak": (_i, [_i, C.POINTER(_d), C.POINTER(_d)]),
@@ -183,6 +184,16 @@ def laplacian_apply(basis, geom, inp, out, stream=None):
 
 def helmholtz_apply(basis, geom, lam, inp, out, stream=None):
     _check(lib.nk_helmholtz_apply(basis.h, geom.h, float(lam), _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+
+
+def helmholtz_apply_fields(basis, geom, lam, inps, outs, stream=None):
+    """inps / outs: sequences of nfields device tensors [nelem][Nm] sharing the geometry of `geom`."""
+    n = len(inps)
+    if n != len(outs):
+        raise ValueError("as many outputs as inputs")
+    pin = (_p * n)(*[_dev_ptr(t) for t in inps])
+    pout = (_p * n)(*[_dev_ptr(t) for t in outs])
+    _check(lib.nk_helmholtz_apply_fields(basis.h, geom.h, float(lam), n, pin, pout, _stream(stream)))
 
 
 def helmholtz_apply_blocks(blocks, lam, stream=None):

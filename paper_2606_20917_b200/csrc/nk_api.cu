@@ -343,7 +343,7 @@ namespace {
 
 nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, int64_t nelem, const double* in0,
                  const double* in1, const double* in2, double* out0, double* out1, double* out2, double lambda,
-                 void* stream)
+                 void* stream, int nfields = 1, const double* const* fin = nullptr, double* const* fout = nullptr)
 {
     if (!b) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": basis is NULL");
     if (op != nk::OP_BWD) {
@@ -358,12 +358,26 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     if ((need_in0 && !in0) || (op != nk::OP_PHYSDERIV && !out0))
         return fail(NK_ERR_INVALID_ARG, std::string(name) + ": NULL field pointer");
     if (in0 && (in0 == out0)) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": in and out alias");
+    if (fin) {
+        for (int f = 0; f < nfields; ++f) {
+            if (!fin[f] || !fout[f]) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": NULL field pointer");
+            for (int h = 0; h < nfields; ++h)
+                if (fin[f] == fout[h]) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": in and out alias");
+            for (int h = 0; h < f; ++h)
+                if (fout[f] == fout[h]) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": two fields share an output");
+        }
+    }
     nk_status st = ensure_device();
     if (st != NK_OK) return st;
     const int E = b->inst->E[(g && g->deformed) ? 1 : 0];
     nk::KArgs a;
     a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
     a.out[0] = out0; a.out[1] = out1; a.out[2] = out2;
+    for (int f = 0; f < nk::K_MAX_FIELDS; ++f) {
+        a.fin[f] = (fin && f < nfields) ? fin[f] : in0;
+        a.fout[f] = (fout && f < nfields) ? fout[f] : out0;
+    }
+    a.nfields = fin ? nfields : 1;
     a.geom = nullptr;
     int def = 0;
     if (g) {
@@ -413,6 +427,15 @@ extern "C" nk_status nk_helmholtz_apply(const nk_basis* b, const nk_geom* g, dou
                                         double* out, void* stream)
 {
     return run_op(nk::OP_HELM, "nk_helmholtz_apply", b, g, 0, in, nullptr, nullptr, out, nullptr, nullptr, lambda, stream);
+}
+
+extern "C" nk_status nk_helmholtz_apply_fields(const nk_basis* b, const nk_geom* g, double lambda, int nfields,
+                                               const double* const* in, double* const* out, void* stream)
+{
+    if (nfields < 1 || nfields > nk::K_MAX_FIELDS || !in || !out)
+        return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_fields: nfields must be 1..8 and the pointer arrays non-NULL");
+    return run_op(nk::OP_HELM, "nk_helmholtz_apply_fields", b, g, 0, in[0], nullptr, nullptr, out[0], nullptr, nullptr, lambda,
+                  stream, nfields, in, out);
 }
 
 extern "C" nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double lambda, void* stream)

@@ -49,7 +49,9 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
         pf_pct = ev ? std::atoi(ev) : 12;
     }
     b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * pf_pct / 100) + 1 : 0x3fffffff;
-    kern<<<a.ngroups, T::NT, smem, stream>>>(tabs, st, b);
+    const long long nblocks = (long long)a.ngroups * (a.nfields > 1 ? a.nfields : 1);
+    if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
+    kern<<<(unsigned)nblocks, T::NT, smem, stream>>>(tabs, st, b);
     return cudaGetLastError();
 }
 

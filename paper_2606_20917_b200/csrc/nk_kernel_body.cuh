@@ -87,7 +87,12 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     // loads of every stage out of such a loop, holds them in registers and spills them (measured: 300 B of
     // spills per thread and a third of the issue slots lost).
     {
-        const int g = blockIdx.x;
+        constexpr bool FIELDS = (OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);
+        const int fld = (FIELDS && a.nfields > 1) ? (int)(blockIdx.x % a.nfields) : 0;
+        const int g = (FIELDS && a.nfields > 1) ? (int)(blockIdx.x / a.nfields) : (int)blockIdx.x;
+        const double* __restrict__ fin0 = FIELDS ? a.fin[fld] : a.in[0];
+        double* __restrict__ fout0 = FIELDS ? a.fout[fld] : a.out[0];
+        (void)fin0; (void)fout0;
         const long long elem = (long long)g * E + e;
         const bool valid = elem < a.nelem;
         const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
@@ -105,7 +110,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             constexpr int NIN = IN_COEFF ? NMODES : NQ;
             const int gn = g + a.pf_dist;
             if (gn < a.ngroups && tid == 32) {
-                const double* base = a.in[0];
+                const double* base = IN_COEFF ? fin0 : a.in[0];
                 if (base && (reinterpret_cast<size_t>(base) & 15) == 0) {
                     const long long e0 = (long long)gn * E;
                     const long long cnt = (a.nelem - e0 < E) ? (a.nelem - e0) : E;
@@ -117,9 +122,9 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
         // ================= input side =================
         if constexpr (IN_COEFF) {
             // a1: coefficients -> Y as C[m]
-            const double* __restrict__ src = a.in[0] + elem * NMODES;
+            const double* __restrict__ src = fin0 + elem * NMODES;
             // LDGSTS (cp.async): every trip in flight at once, no registers held, zero-fill for the ragged tail
-            NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : a.in[0], valid);
+            NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : fin0, valid);
             cp_async_wait_all();
             __syncthreads();
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z

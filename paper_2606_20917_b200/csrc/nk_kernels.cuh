@@ -123,9 +123,16 @@ struct SimplexTabsFor {
     using type = SimplexTabs<(SHAPE == K_HEX) ? 1 : (NM * (NM + 1) / 2) * Q>;
 };
 
+enum { K_MAX_FIELDS = 8 };
 struct KArgs {
     const double* in[3];
     double* out[3];
+    // multi-field blocks: nfields coefficient fields share one geometry.  Block b works on group
+    // b / nfields of field b % nfields: the blocks of one group are neighbours in launch order, run at the
+    // same time, and the geometry is read from DRAM once and from L2 by the others.
+    const double* fin[K_MAX_FIELDS];
+    double* fout[K_MAX_FIELDS];
+    int nfields;             // 1 for the single-field calls (then fin[0] == in[0], fout[0] == out[0])
     const double* geom;      // metric stream (7 comps) or factor stream (10 comps), see nk_api.cu
     double lambda;
     long long nelem;

@@ -165,3 +165,33 @@ def test_helmholtz_host_entry(nk):
     assert nk.launch_count() == n0 + 1
     ref = o.helmholtz(el, A.numpy(), J.numpy(), 1.0, x.numpy())
     assert K.normwise_err(y.numpy(), ref) <= TOL
+
+
+@pytest.mark.parametrize("shape,deformed", [(o.HEX, True), (o.TET, False), (o.PRISM, True)])
+def test_helmholtz_fields(nk, shape, deformed):
+    """nk_helmholtz_apply_fields (multi-field block): each field equals the oracle's Helmholtz of that
+    field, and is bit-identical to the single-field call."""
+    P, lam, nf = 3, 2.5, 3
+    el = K.element(shape, P)
+    full = K.mesh(shape, 3)[0].shape[0]
+    A, J = K.geometry(shape, P, 3, deformed, take=torch.arange(full - 3))
+    ne = J.shape[0]
+    basis = nk.Basis(shape, P)
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), deformed)
+    xs = [wl.coefficients(100 + f, ne, el.Nm) for f in range(nf)]
+    dx = [x.cuda() for x in xs]
+    dy = [torch.full_like(x, float("nan")) for x in dx]
+    n0 = nk.launch_count()
+    nk.helmholtz_apply_fields(basis, geom, lam, dx, dy)
+    assert nk.launch_count() == n0 + 1          # ONE launch for all fields
+    torch.cuda.synchronize()
+    for f in range(nf):
+        ref = o.helmholtz(el, A.numpy(), J.numpy(), lam, xs[f].numpy())
+        assert K.normwise_err(dy[f].cpu().numpy(), ref) <= TOL
+        y1 = torch.empty_like(dx[f])
+        nk.helmholtz_apply(basis, geom, lam, dx[f], y1)
+        assert torch.equal(y1, dy[f])
+    with pytest.raises(nk.NkError):
+        nk.helmholtz_apply_fields(basis, geom, lam, dx, [dy[0], dy[0], dy[2]])
+    with pytest.raises(nk.NkError):
+        nk.helmholtz_apply_fields(basis, geom, lam, dx, [dy[0], dx[1], dy[2]])
