@@ -46,7 +46,7 @@ struct Tune {
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = DEF ? (Q <= 3 ? 16 : Q <= 5 ? 8 : Q <= 8 ? 4 : 2)
+    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : 2)
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
