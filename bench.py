@@ -2,7 +2,7 @@
 """bench.py -- Helmholtz-apply throughput (GDoF/s, fp64) of libnk on B200, with the roofline fraction of
 the kernel and the CPU oracle timed beside it.  Contract: see DESIGN.md section 8.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2[:P]|cfg3[:P]|cfg4:P|cfg5] [--impl reference]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2[:P]|cfg3[:P]|cfg4:P|cfg5[:P]] [--impl reference]
 
 A step = one pass of the whole hot path (ONE fused kernel per block) over the
 workload's mesh.  N > 1 (torchrun): every rank owns a mesh of the same size (elements are independent,
@@ -42,7 +42,7 @@ def parse_args():
 
 
 def workload_blocks(name, device, rank=0):
-    P = int(name.split(":")[1]) if ":" in name else None       # cfg4:P (and cfg2:P, cfg3:P): the P-sweep
+    P = int(name.split(":")[1]) if ":" in name else None       # cfg4:P (and cfg2:P, cfg3:P, cfg5:P): the P-sweep
     title, op, blocks = cfgs.config_blocks(int(name[3:4]), device=device, P_sweep=P)
     for b in blocks:
         b["seed"] += 1000 * rank

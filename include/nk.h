@@ -136,7 +136,10 @@ nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double 
 
 /* End-to-end variant with HOST field buffers: copies host_in to an internal device buffer, applies the
  * Helmholtz operator and copies the result back into host_out; synchronises `stream` before returning.
- * Pinned host memory makes the copies asynchronous DMA; pageable memory works but is slower.         */
+ * The work is cut into up to 8 chunks of element groups and pipelined over two internal copy streams, so that
+ * the host-to-device copy of one chunk, the kernel of the previous one and the device-to-host copy of the one
+ * before overlap (PCIe is full duplex).  Pinned host memory is needed for the overlap; pageable memory works
+ * but serialises.                                                                                   */
 nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g, double lambda, const double* host_in,
                                   double* host_out, void* stream);
 

@@ -1,5 +1,6 @@
 // nk_api.cu -- the C-ABI of include/nk.h (layer B3), the dispatcher (B1), the geometry repack
 // kernels and the fp64 probe.  No torch types, no CPU fallback.
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -76,8 +77,12 @@ struct nk_geom {
     int deformed = 0, E = 1;
     double* d_metric = nullptr; // [group][7][npt][E]
     double* d_factor = nullptr; // [group][10][npt][E]
+    // nk_helmholtz_apply_host: device staging buffers and the copy-in / copy-out pipeline
     double* d_stage_in = nullptr;
     double* d_stage_out = nullptr;
+    enum { kChunks = 8 };
+    cudaStream_t s_in = nullptr, s_out = nullptr;
+    cudaEvent_t ev_start = nullptr, ev_done = nullptr, ev_in[kChunks] = {}, ev_k[kChunks] = {};
 };
 
 // =========================== basis ===========================
@@ -332,6 +337,14 @@ extern "C" nk_status nk_geom_destroy(nk_geom* g)
     if (g->d_factor) cudaFree(g->d_factor);
     if (g->d_stage_in) cudaFree(g->d_stage_in);
     if (g->d_stage_out) cudaFree(g->d_stage_out);
+    if (g->s_in) cudaStreamDestroy(g->s_in);
+    if (g->s_out) cudaStreamDestroy(g->s_out);
+    if (g->ev_start) cudaEventDestroy(g->ev_start);
+    if (g->ev_done) cudaEventDestroy(g->ev_done);
+    for (int c = 0; c < nk_geom::kChunks; ++c) {
+        if (g->ev_in[c]) cudaEventDestroy(g->ev_in[c]);
+        if (g->ev_k[c]) cudaEventDestroy(g->ev_k[c]);
+    }
     delete g;
     return NK_OK;
 }
@@ -343,7 +356,8 @@ namespace {
 
 nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, int64_t nelem, const double* in0,
                  const double* in1, const double* in2, double* out0, double* out1, double* out2, double lambda,
-                 void* stream, int nfields = 1, const double* const* fin = nullptr, double* const* fout = nullptr)
+                 void* stream, int nfields = 1, const double* const* fin = nullptr, double* const* fout = nullptr,
+                 int64_t group0 = 0, int64_t group_count = -1)
 {
     if (!b) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": basis is NULL");
     if (op != nk::OP_BWD) {
@@ -389,6 +403,9 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     const int64_t ngroups = (nelem + E - 1) / E;
     if (ngroups > 0x7fffffffLL) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": too many elements");
     a.ngroups = (int)ngroups;
+    a.g0 = (int)group0;
+    a.grid_groups = (int)(group_count < 0 ? ngroups : group_count);
+    if (a.g0 < 0 || a.g0 + (int64_t)a.grid_groups > ngroups) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": bad group range");
     cudaError_t e = b->inst->fn[def][op](b->tabs_flat.data(), b->sx_flat.data(), a, g_num_sms, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, name);
     { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
@@ -462,13 +479,47 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
         if (e != cudaSuccess) { g_err = "nk_helmholtz_apply_host: cudaMalloc failed"; return NK_ERR_ALLOC; }
     }
     cudaStream_t s = (cudaStream_t)stream;
-    e = cudaMemcpyAsync(g->d_stage_in, host_in, bytes, cudaMemcpyHostToDevice, s);
-    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: H2D");
-    nk_status st = nk_helmholtz_apply(b, g, lambda, g->d_stage_in, g->d_stage_out, stream);
-    if (st != NK_OK) return st;
-    e = cudaMemcpyAsync(host_out, g->d_stage_out, bytes, cudaMemcpyDeviceToHost, s);
+    // Pipeline over chunks of groups: H2D on s_in, the fused kernel on the caller's stream, D2H on s_out, chained
+    // by events, so that the copy-in of chunk c+1 and the copy-out of chunk c-1 (PCIe is full duplex) overlap
+    // the kernel of chunk c.  One cudaMemcpyAsync per chunk and direction.
+    if (!g->s_in) {
+        e = cudaStreamCreateWithFlags(&g->s_in, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&g->s_out, cudaStreamNonBlocking);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->ev_start, cudaEventDisableTiming);
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->ev_done, cudaEventDisableTiming);
+        for (int c = 0; c < nk_geom::kChunks && e == cudaSuccess; ++c) {
+            e = cudaEventCreateWithFlags(&g->ev_in[c], cudaEventDisableTiming);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->ev_k[c], cudaEventDisableTiming);
+        }
+        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: stream / event creation");
+    }
+    const int64_t per = (g->ngroups + nk_geom::kChunks - 1) / nk_geom::kChunks;
+    const size_t elem_bytes = (size_t)b->t.Nm * sizeof(double);
+    e = cudaEventRecord(g->ev_start, s);                  // order after the caller's earlier work on `stream`
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_in, g->ev_start, 0);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_out, g->ev_start, 0);
+    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: pipeline start");
+    for (int c = 0; c < nk_geom::kChunks; ++c) {
+        const int64_t g0 = c * per, g1 = std::min<int64_t>(g->ngroups, g0 + per);
+        if (g0 >= g1) break;
+        const int64_t e0 = g0 * g->E, e1 = std::min<int64_t>(g->nelem, g1 * g->E);
+        const size_t off = (size_t)e0 * b->t.Nm, nb = (size_t)(e1 - e0) * elem_bytes;
+        e = cudaMemcpyAsync(g->d_stage_in + off, host_in + off, nb, cudaMemcpyHostToDevice, g->s_in);
+        if (e == cudaSuccess) e = cudaEventRecord(g->ev_in[c], g->s_in);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, g->ev_in[c], 0);
+        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: H2D");
+        nk_status st = run_op(nk::OP_HELM, "nk_helmholtz_apply_host", b, g, 0, g->d_stage_in, nullptr, nullptr, g->d_stage_out,
+                              nullptr, nullptr, lambda, stream, 1, nullptr, nullptr, g0, g1 - g0);
+        if (st != NK_OK) return st;
+        e = cudaEventRecord(g->ev_k[c], s);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_out, g->ev_k[c], 0);
+        if (e == cudaSuccess) e = cudaMemcpyAsync(host_out + off, g->d_stage_out + off, nb, cudaMemcpyDeviceToHost, g->s_out);
+        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: D2H");
+    }
+    e = cudaEventRecord(g->ev_done, g->s_out);
+    if (e == cudaSuccess) e = cudaStreamWaitEvent(s, g->ev_done, 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: D2H");
+    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: synchronise");
     return NK_OK;
 }
 

@@ -38,7 +38,7 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
         if (err != cudaSuccess) return err;
         blocks_per_sm = bps < 1 ? 1 : bps;
     }
-    if (a.ngroups <= 0) return cudaSuccess;
+    if (a.grid_groups <= 0) return cudaSuccess;
     KArgs b = a;
     // L2 prefetch distance = 1/8 of the co-resident blocks (B200 sweep, profiles/r1_notes.md: flat between 3 %
     // and 25 %; at 100 % a third of the prefetched lines are evicted before use and re-read from DRAM).
@@ -49,7 +49,7 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
         pf_pct = ev ? std::atoi(ev) : 12;
     }
     b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * pf_pct / 100) + 1 : 0x3fffffff;
-    const long long nblocks = (long long)a.ngroups * (a.nfields > 1 ? a.nfields : 1);
+    const long long nblocks = (long long)a.grid_groups * (a.nfields > 1 ? a.nfields : 1);
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     kern<<<(unsigned)nblocks, T::NT, smem, stream>>>(tabs, st, b);
     return cudaGetLastError();

@@ -89,7 +89,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     {
         constexpr bool FIELDS = (OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);
         const int fld = (FIELDS && a.nfields > 1) ? (int)(blockIdx.x % a.nfields) : 0;
-        const int g = (FIELDS && a.nfields > 1) ? (int)(blockIdx.x / a.nfields) : (int)blockIdx.x;
+        const int g = a.g0 + ((FIELDS && a.nfields > 1) ? (int)(blockIdx.x / a.nfields) : (int)blockIdx.x);
         const double* __restrict__ fin0 = FIELDS ? a.fin[fld] : a.in[0];
         double* __restrict__ fout0 = FIELDS ? a.fout[fld] : a.out[0];
         (void)fin0; (void)fout0;

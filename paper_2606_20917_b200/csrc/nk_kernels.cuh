@@ -136,7 +136,8 @@ struct KArgs {
     const double* geom;      // metric stream (7 comps) or factor stream (10 comps), see nk_api.cu
     double lambda;
     long long nelem;
-    int ngroups;
+    int ngroups;             // groups of the whole block of elements
+    int g0, grid_groups;     // this launch works on groups [g0, g0 + grid_groups) (chunked host pipeline)
     int pf_dist;             // L2 prefetch distance in groups = number of co-resident blocks
 };
 

@@ -42,13 +42,16 @@ def config_blocks(cfg, device="cpu", P_sweep=None, scale=1.0):
         return ("cfg4 hex affine P%d Q%d, %d^3 el" % (P_sweep, P_sweep + 2, n), "mass+laplacian",
                 [dict(shape=HEX, P=P_sweep, lam=0.0, deformed=False, v0=v0, E=E, seed=seed)])
     if cfg == 5:
-        n = max(4, int(round(40 * scale)))
+        P = 5 if P_sweep is None else P_sweep
+        # other orders: cube count chosen to keep the geometry stream of the P=5 case (3.7 GB)
+        n0 = 40 if P == 5 else 40 * 7.0 / (P + 2)
+        n = max(4, int(round(n0 * scale)))
         zt = max(1, n // 4)                       # z-layers 0..n/4-1 -> tets, the rest -> prisms
         vt, Et = wl.kuhn_tet_mesh(n, 0, zt, device=device)
         vp, Ep = wl.prism_mesh(n, zt, n, device=device)
-        return ("cfg5 hybrid deformed P5 Q7, %d tets + %d prisms" % (vt.shape[0], vp.shape[0]), "helmholtz",
-                [dict(shape=PRISM, P=5, lam=10.0, deformed=True, v0=vp, E=Ep, seed=seed),
-                 dict(shape=TET, P=5, lam=10.0, deformed=True, v0=vt, E=Et, seed=seed + 100)])
+        return ("cfg5 hybrid deformed P%d Q%d, %d tets + %d prisms" % (P, P + 2, vt.shape[0], vp.shape[0]), "helmholtz",
+                [dict(shape=PRISM, P=P, lam=10.0, deformed=True, v0=vp, E=Ep, seed=seed),
+                 dict(shape=TET, P=P, lam=10.0, deformed=True, v0=vt, E=Et, seed=seed + 100)])
     raise ValueError("config 1..5")
 
 
