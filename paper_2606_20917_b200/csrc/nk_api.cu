@@ -451,7 +451,7 @@ extern "C" nk_status nk_helmholtz_apply_fields(const nk_basis* b, const nk_geom*
 {
     if (nfields < 1 || nfields > nk::K_MAX_FIELDS || !in || !out)
         return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_fields: nfields must be 1..8 and the pointer arrays non-NULL");
-    return run_op(nk::OP_HELM, "nk_helmholtz_apply_fields", b, g, 0, in[0], nullptr, nullptr, out[0], nullptr, nullptr, lambda,
+    return run_op(nfields > 1 ? nk::OP_HELMF : nk::OP_HELM, "nk_helmholtz_apply_fields", b, g, 0, in[0], nullptr, nullptr, out[0], nullptr, nullptr, lambda,
                   stream, nfields, in, out);
 }
 

@@ -60,7 +60,7 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
         launch<NK_SHAPE, NK_P, DEF, OP_BWD>, launch<NK_SHAPE, NK_P, DEF, OP_IPROD>,                     \
             launch<NK_SHAPE, NK_P, DEF, OP_PHYSDERIV>, launch<NK_SHAPE, NK_P, DEF, OP_IPDERIV>,         \
             launch<NK_SHAPE, NK_P, DEF, OP_MASS>, launch<NK_SHAPE, NK_P, DEF, OP_LAP>,                  \
-            launch<NK_SHAPE, NK_P, DEF, OP_HELM>                                                        \
+            launch<NK_SHAPE, NK_P, DEF, OP_HELM>, launch<NK_SHAPE, NK_P, DEF, OP_HELMF>                 \
     }
 
 } // namespace nk

@@ -49,12 +49,13 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, 
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-template <int SHAPE, int P, int DEF, int OP>
+template <int SHAPE, int P, int DEF, int OPX>
 __global__ void __launch_bounds__(Tune<SHAPE, P, DEF>::NT, Tune<SHAPE, P, DEF>::MINB)
 nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
           const __grid_constant__ typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st, const __grid_constant__ KArgs a)
 {
     using T = Tune<SHAPE, P, DEF>;
+    constexpr int OP = (OPX == OP_HELMF) ? OP_HELM : OPX;
     constexpr int NM = P + 1, Q = P + 2, E = T::E, LS = T::LS, LQ = T::LQ;
     constexpr int NQ = Q * Q * Q, NQP = T::NQP, NMODES = k_num_modes(SHAPE, NM);
     constexpr bool IN_COEFF = (OP == OP_BWD || OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);
@@ -87,12 +88,12 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     // loads of every stage out of such a loop, holds them in registers and spills them (measured: 300 B of
     // spills per thread and a third of the issue slots lost).
     {
-        constexpr bool FIELDS = (OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);
+        constexpr bool FIELDS = (OPX == OP_HELMF);
         const int fld = (FIELDS && a.nfields > 1) ? (int)(blockIdx.x % a.nfields) : 0;
         const int g = a.g0 + ((FIELDS && a.nfields > 1) ? (int)(blockIdx.x / a.nfields) : (int)blockIdx.x);
-        const double* __restrict__ fin0 = FIELDS ? a.fin[fld] : a.in[0];
-        double* __restrict__ fout0 = FIELDS ? a.fout[fld] : a.out[0];
-        (void)fin0; (void)fout0;
+        // field pointers are re-read from the parameter bank where they are used (no registers held across stages)
+#define NK_FIN0 (FIELDS ? a.fin[fld] : a.in[0])
+#define NK_FOUT0 (FIELDS ? a.fout[fld] : a.out[0])
         const long long elem = (long long)g * E + e;
         const bool valid = elem < a.nelem;
         const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
@@ -110,7 +111,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             constexpr int NIN = IN_COEFF ? NMODES : NQ;
             const int gn = g + a.pf_dist;
             if (gn < a.ngroups && tid == 32) {
-                const double* base = IN_COEFF ? fin0 : a.in[0];
+                const double* base = IN_COEFF ? NK_FIN0 : a.in[0];
                 if (base && (reinterpret_cast<size_t>(base) & 15) == 0) {
                     const long long e0 = (long long)gn * E;
                     const long long cnt = (a.nelem - e0 < E) ? (a.nelem - e0) : E;
@@ -122,9 +123,9 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
         // ================= input side =================
         if constexpr (IN_COEFF) {
             // a1: coefficients -> Y as C[m]
-            const double* __restrict__ src = fin0 + elem * NMODES;
+            const double* __restrict__ src = NK_FIN0 + elem * NMODES;
             // LDGSTS (cp.async): every trip in flight at once, no registers held, zero-fill for the ragged tail
-            NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : fin0, valid);
+            NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : NK_FIN0, valid);
             cp_async_wait_all();
             __syncthreads();
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
@@ -169,6 +170,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
 #include "nk_stage_mid.inc"
 #include "nk_stage_out.inc"
     }
+#undef NK_FIN0
+#undef NK_FOUT0
 #undef GIDX
 #undef T1IDX
 #undef T2IDX

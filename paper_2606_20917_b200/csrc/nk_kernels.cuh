@@ -26,7 +26,9 @@
 namespace nk {
 
 enum { K_HEX = 0, K_TET = 1, K_PRISM = 2 };
-enum { OP_BWD = 0, OP_IPROD, OP_PHYSDERIV, OP_IPDERIV, OP_MASS, OP_LAP, OP_HELM, OP_COUNT };
+// OP_HELMF = OP_HELM on a multi-field block (its own instantiation: the field bookkeeping costs the
+// single-field affine kernels 6 % at their 64-register budget)
+enum { OP_BWD = 0, OP_IPROD, OP_PHYSDERIV, OP_IPDERIV, OP_MASS, OP_LAP, OP_HELM, OP_HELMF, OP_COUNT };
 
 __host__ __device__ constexpr int k_num_modes(int shape, int nm)
 {
