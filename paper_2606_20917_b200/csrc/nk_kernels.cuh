@@ -48,7 +48,7 @@ struct Tune {
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : 2)
+    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : 4)
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
