@@ -99,3 +99,52 @@ def test_config4_full_size_sampled(nk, P):
     An, Jn, xn = A[idx].cpu().numpy(), J[idx].cpu().numpy(), x[idx].cpu().numpy()
     assert K.normwise_err(ym[idx].cpu().numpy(), o.mass(el, Jn, xn)) <= TOL
     assert K.normwise_err(yl[idx].cpu().numpy(), o.laplacian(el, An, Jn, xn)) <= TOL
+
+
+def _ones(basis, ne, dev):
+    """coefficients of the constant function 1: the vertex modes (A8: they sum to 1)."""
+    verts = {0: [(p, q, r) for p in (0, 1) for q in (0, 1) for r in (0, 1)],
+             1: [(0, 0, 0), (1, 0, 0), (0, 1, 0), (0, 0, 1)],
+             2: [(0, 0, 0), (1, 0, 0), (0, 1, 0), (1, 1, 0), (0, 0, 1), (0, 1, 1)]}[basis.shape]
+    one = torch.zeros((ne, basis.num_modes), dtype=torch.float64, device=dev)
+    for v in verts:
+        m = basis.mode_index(*v)
+        assert m >= 0
+        one[:, m] = 1.0
+    return one
+
+
+@pytest.mark.parametrize("cfg", [2, 3, 5])
+def test_full_size_invariants_all_elements(nk, cfg):
+    """Properties that hold at any size, checked on EVERY element of the BASELINE meshes (north_star
+    invariants): integrating 1 gives the volume of the unit cube; the Laplacian annihilates constants;
+    the Helmholtz operator is symmetric."""
+    dev = torch.device("cuda", 0)
+    title, op, blocks = cfgs.config_blocks(cfg, device=dev)
+    vol = 0.0
+    for b in blocks:
+        basis = nk.Basis(b["shape"], b["P"])
+        A, J = cfgs.block_factors(b, basis.points())
+        geom = nk.Geom(basis, A, J, b["deformed"])
+        ne = J.shape[0]
+        del A, J
+        one = _ones(basis, ne, dev)
+        y = torch.empty_like(one)
+        nk.mass_apply(basis, geom, one, y)
+        vol += float((one * y).sum())
+        x = wl.coefficients(b["seed"], ne, basis.num_modes).to(dev)
+        z = wl.coefficients(b["seed"] + 1, ne, basis.num_modes).to(dev)
+        lx = torch.empty_like(x)
+        nk.laplacian_apply(basis, geom, x, lx)
+        nk.laplacian_apply(basis, geom, one, y)
+        scale = lx.abs().amax(dim=1)
+        assert float((y.abs().amax(dim=1) / scale).max()) <= 1e-12, "L 1 != 0 (%s)" % title
+        hx, hz = torch.empty_like(x), torch.empty_like(x)
+        nk.helmholtz_apply(basis, geom, b["lam"], x, hx)
+        nk.helmholtz_apply(basis, geom, b["lam"], z, hz)
+        a1, a2 = (z * hx).sum(dim=1), (x * hz).sum(dim=1)           # per element: <z, H x> = <x, H z>
+        den = (z.abs() * hx.abs()).sum(dim=1)
+        assert float(((a1 - a2).abs() / den).max()) <= 1e-12, "H not symmetric (%s)" % title
+    # config 5: the tets fill z in [0, 1/4) and the prisms the rest, together the unit cube
+    tol = 1e-9 if blocks[0]["deformed"] else 1e-12     # the sinusoidal map integrates to 1 up to quadrature error
+    assert abs(vol - 1.0) <= tol, "sum of element volumes %.15g (%s)" % (vol, title)
