@@ -4,16 +4,18 @@
 // Design:
 //   * a thread block works on a GROUP of E elements at a time; all on-chip arrays are
 //     element-interleaved, index = idx*E + e, thread = (e = tid % E, slot = tid / E).
-//     A half-warp therefore touches E consecutive doubles per line: shared-memory accesses
-//     are conflict-free by construction and the geometry stream (stored in the same
-//     interleaved order) is read as fully coalesced 256-byte warp loads.
+//     A half-warp therefore touches E consecutive doubles of 16/E lines whose strides are odd
+//     multiples of E: conflict-free when 16/E divides Q (a few two-way conflicts otherwise); the
+//     geometry stream (stored in the same interleaved order) is read as full 32-byte sectors.
+//     One block = one group (grid = number of groups): a persistent loop makes ptxas hoist and
+//     spill the constant-bank matrices.
 //   * every tensor contraction is "one thread per quadrature LINE": the thread pulls one
 //     line of one element into registers and contracts it with a 1-D matrix whose entries
 //     are compile-time-indexed kernel parameters, i.e. constant-bank operands of DFMA --
 //     no shared-memory traffic for the basis / derivative matrices (Eq. 16, 20, 22).
-//   * the simplex contractions with triangular bounds (Eq. 17, 21) run from host-built
-//     index arrays staged once per block in shared memory; the C0 corrections
-//     of A8 are ordinary entries of those arrays.
+//   * the simplex contractions with triangular bounds (Eq. 17, 21) give each warp one class
+//     of lines, so that bounds and psi^b rows are warp-uniform compile-time constants
+//     (nk_stage_sx.inc); the C0 corrections of A8 are compile-time special cases.
 //   * the Helmholtz chain (a1..a9 of SURVEY 8(a)) is fused: three shared arrays X, Y, Z of
 //     Q^3*E doubles are reused by a static plan (cf. the buffer-reuse pass);
 //     quadrature-point data never goes to HBM.
