@@ -215,6 +215,9 @@ def main():
         ys = [torch.empty_like(xs[0]) for _ in range(NSETS)]
         work.append((basis, geom, xs, ys, b["lam"], ne))
         by, fl = algorithmic(b["shape"], b["P"], b["deformed"], "helmholtz")
+        if op == "mass+laplacian":          # config 4: one mass and one Laplacian launch per step
+            bm, fm = algorithmic(b["shape"], b["P"], b["deformed"], "mass")
+            by, fl = by + bm, fl - 2 * basis.num_points + fm
         nf = args.fields
         dof += ne * basis.num_modes * nf
         alg_bytes += (by + 16 * basis.num_modes * (nf - 1)) * ne      # the geometry is shared by the fields
@@ -278,6 +281,29 @@ def main():
     ms_step = ms_total / args.steps
     value = dof * world / (ms_step * 1e-3) / 1e9
 
+    # ---- config 4: mass and Laplacian timed separately (locates the bandwidth / compute crossover) ----
+    per_op = None
+    if op == "mass+laplacian":
+        per_op = {}
+        basis, geom, xs, ys, _, ne = work[0]
+        b0 = blocks[0]
+        for name, fn in (("mass", nk.mass_apply), ("laplacian", nk.laplacian_apply)):
+            for i in range(3):
+                fn(basis, geom, xs[i % NSETS], ys[i % NSETS])
+            barrier()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record()
+            for i in range(args.steps):
+                fn(basis, geom, xs[i % NSETS], ys[i % NSETS])
+            t1.record()
+            barrier()
+            ms1 = t0.elapsed_time(t1) / args.steps
+            bb, ff = algorithmic(b0["shape"], b0["P"], b0["deformed"], "mass" if name == "mass" else "helmholtz")
+            if name == "laplacian":
+                ff -= 2 * basis.num_points
+            per_op[name] = {"ms": ms1, "gdofs": ne * basis.num_modes / (ms1 * 1e-3) / 1e9,
+                            "alg_gbs": bb * ne / (ms1 * 1e-3) / 1e9, "alg_tflops": ff * ne / (ms1 * 1e-3) / 1e12}
+
     # ---- end to end: HOST buffers through nk_helmholtz_apply_host (H2D + kernel + D2H per step) ----
     e2e = None
     if op == "helmholtz" and args.fields == 1:
@@ -338,6 +364,10 @@ def main():
     else:
         roof = {"bound": "alu", "achieved": ach_tf, "peak": fp64_tf, "unit": "TFLOP/s", "frac": fp_frac,
                 "traffic": traffic, "peak_source": "nk_probe_fp64_peak (register-only DFMA chains, this run)"}
+    if per_op:
+        for v in per_op.values():
+            v["hbm_frac"], v["fp64_frac"] = v.pop("alg_gbs") / hbm_peak, v.pop("alg_tflops") / fp64_tf
+        roof["per_op"] = per_op
     roof["other"] = {"hbm_frac": hbm_frac, "fp64_frac": fp_frac, "fp64_probe_tflops": fp64_tf,
                      "fp64_nominal_tflops": FP64_NOMINAL_TFLOPS, "algorithmic_bytes_per_launch": alg_bytes,
                      "algorithmic_flops_per_launch": alg_flops, "kernel_ms": ms_step / max(1, launches // args.steps)}
