@@ -15,3 +15,17 @@ def pytest_configure(config):
 @pytest.fixture(scope="session")
 def repo_root():
     return ROOT
+
+
+def pytest_sessionstart(session):
+    """Build libnk.so (incrementally, in-tree) before the tests import it, so that a fresh checkout or an
+    edited kernel is never tested against a stale or missing library.  Without nvcc the CPU tests of the
+    library skip themselves and the GPU tests fail loudly at import (there is no CPU fallback)."""
+    import shutil
+    if not (shutil.which("nvcc") or os.path.exists("/usr/local/cuda/bin/nvcc")):
+        return
+    try:
+        from paper_2606_20917_b200 import build as _b
+        _b.build()
+    except Exception as exc:   # the import of the binding reports the real problem
+        print("libnk build failed: %s" % exc, file=sys.stderr)
