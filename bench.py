@@ -208,7 +208,7 @@ def main():
     for b in blocks:
         basis = nk.Basis(b["shape"], b["P"])
         A, J = cfgs.block_factors(b, basis.points())
-        geom = nk.Geom(basis, A, J, b["deformed"])
+        geom = nk.Geom(basis, A, J, b["deformed"], streams=nk.Geom.METRIC)
         ne = J.shape[0]
         del A, J
         xs = [wl.coefficients(b["seed"] + s, ne, basis.num_modes).to(dev) for s in range(NSETS)]

@@ -93,6 +93,13 @@ int nk_basis_mode_index(const nk_basis* b, int p, int q, int r);
  * deformed.  nelem == 0 is valid (every apply is then a no-op).                                      */
 nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
                          const double* detJ, int on_device, void* stream, nk_geom** out);
+/* The same, building only the streams asked for (a Helmholtz-only caller saves 10 of 17 doubles per point):
+ * NK_GEOM_METRIC serves nk_iprod, nk_mass_apply, nk_laplacian_apply and every nk_helmholtz_* call,
+ * NK_GEOM_FACTORS serves nk_physderiv and nk_iprod_deriv.  An operator whose stream is missing returns
+ * NK_ERR_INVALID_ARG.  nk_geom_upload builds both.                                                    */
+enum { NK_GEOM_METRIC = 1, NK_GEOM_FACTORS = 2 };
+nk_status nk_geom_upload_streams(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
+                                 const double* detJ, int on_device, unsigned streams, void* stream, nk_geom** out);
 nk_status nk_geom_destroy(nk_geom* g);
 int64_t nk_geom_num_elements(const nk_geom* g);
 

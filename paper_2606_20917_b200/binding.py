@@ -29,6 +29,7 @@ _SIG = {
     "nk_basis_mode_index": (_i, [_p, _i, _i, _i]),
     "nk_basis_get_points": (_i, [_p, C.POINTER(_d), _sz]),
     "nk_geom_upload": (_i, [_p, _i64, _i, _p, _p, _i, _p, C.POINTER(_p)]),
+    "nk_geom_upload_streams": (_i, [_p, _i64, _i, _p, _p, _i, C.c_uint, _p, C.POINTER(_p)]),
     "nk_geom_destroy": (_i, [_p]),
     "nk_geom_num_elements": (_i64, [_p]),
     "nk_bwdtrans": (_i, [_p, _i64, _p, _p, _p]),
@@ -132,7 +133,9 @@ class Basis:
 class Geom:
     """nk_geom handle.  dxi_dx [nelem][npt][3][3], detJ [nelem][npt]; host or device tensors."""
 
-    def __init__(self, basis, dxi_dx, detJ, deformed, stream=None):
+    METRIC, FACTORS = 1, 2
+
+    def __init__(self, basis, dxi_dx, detJ, deformed, stream=None, streams=3):
         nelem = detJ.shape[0]
         npt = basis.num_points if deformed else 1
         if tuple(dxi_dx.shape) != (nelem, npt, 3, 3) or tuple(detJ.shape) != (nelem, npt):
@@ -140,8 +143,8 @@ class Geom:
         if dxi_dx.is_cuda != detJ.is_cuda:
             raise ValueError("dxi_dx and detJ must live on the same side")
         h = _p()
-        _check(lib.nk_geom_upload(basis.h, nelem, int(bool(deformed)), _ptr(dxi_dx), _ptr(detJ),
-                                  int(dxi_dx.is_cuda), _stream(stream), C.byref(h)))
+        _check(lib.nk_geom_upload_streams(basis.h, nelem, int(bool(deformed)), _ptr(dxi_dx), _ptr(detJ),
+                                          int(dxi_dx.is_cuda), int(streams), _stream(stream), C.byref(h)))
         self.h, self.basis, self.nelem, self.deformed = h, basis, nelem, bool(deformed)
 
     def close(self):

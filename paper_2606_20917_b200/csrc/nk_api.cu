@@ -248,10 +248,14 @@ __global__ void repack_kernel(const __grid_constant__ RepackTabs rt, const doubl
         G[3] = wJ * (A[3] * A[3] + A[4] * A[4] + A[5] * A[5]);
         G[4] = wJ * (A[3] * A[6] + A[4] * A[7] + A[5] * A[8]);
         G[5] = wJ * (A[6] * A[6] + A[7] * A[7] + A[8] * A[8]);
-        for (int c = 0; c < 6; ++c) metric[((g * 7 + c) * npt + n) * E + e] = G[c];
-        metric[((g * 7 + 6) * npt + n) * E + e] = wJ;
-        for (int c = 0; c < 9; ++c) factor[((g * 10 + c) * npt + n) * E + e] = A[c];
-        factor[((g * 10 + 9) * npt + n) * E + e] = wJ;
+        if (metric) {
+            for (int c = 0; c < 6; ++c) metric[((g * 7 + c) * npt + n) * E + e] = G[c];
+            metric[((g * 7 + 6) * npt + n) * E + e] = wJ;
+        }
+        if (factor) {
+            for (int c = 0; c < 9; ++c) factor[((g * 10 + c) * npt + n) * E + e] = A[c];
+            factor[((g * 10 + 9) * npt + n) * E + e] = wJ;
+        }
     }
 }
 
@@ -260,6 +264,14 @@ __global__ void repack_kernel(const __grid_constant__ RepackTabs rt, const doubl
 extern "C" nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
                                     const double* detJ, int on_device, void* stream, nk_geom** out)
 {
+    return nk_geom_upload_streams(b, nelem, deformed, dxi_dx, detJ, on_device, NK_GEOM_METRIC | NK_GEOM_FACTORS, stream, out);
+}
+
+extern "C" nk_status nk_geom_upload_streams(const nk_basis* b, int64_t nelem, int deformed, const double* dxi_dx,
+                                            const double* detJ, int on_device, unsigned streams, void* stream, nk_geom** out)
+{
+    if ((streams & (NK_GEOM_METRIC | NK_GEOM_FACTORS)) == 0 || (streams & ~(unsigned)(NK_GEOM_METRIC | NK_GEOM_FACTORS)))
+        return fail(NK_ERR_INVALID_ARG, "nk_geom_upload_streams: streams must be a combination of NK_GEOM_METRIC and NK_GEOM_FACTORS");
     if (!out) return fail(NK_ERR_INVALID_ARG, "nk_geom_upload: out is NULL");
     *out = nullptr;
     if (!b || nelem < 0 || (nelem > 0 && (!dxi_dx || !detJ))) return fail(NK_ERR_INVALID_ARG, "nk_geom_upload: bad arguments");
@@ -277,8 +289,9 @@ extern "C" nk_status nk_geom_upload(const nk_basis* b, int64_t nelem, int deform
     if (nelem == 0) return NK_OK;
     const long long npt = g->deformed ? b->t.Nq : 1;
     const size_t slots = (size_t)g->ngroups * npt * g->E;
-    cudaError_t e = cudaMalloc(&g->d_metric, slots * 7 * sizeof(double));
-    if (e == cudaSuccess) e = cudaMalloc(&g->d_factor, slots * 10 * sizeof(double));
+    cudaError_t e = cudaSuccess;
+    if (streams & NK_GEOM_METRIC) e = cudaMalloc(&g->d_metric, slots * 7 * sizeof(double));
+    if (e == cudaSuccess && (streams & NK_GEOM_FACTORS)) e = cudaMalloc(&g->d_factor, slots * 10 * sizeof(double));
     if (e != cudaSuccess) {
         nk_geom_destroy(g);
         *out = nullptr;
@@ -397,6 +410,9 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     if (g) {
         def = g->deformed;
         a.geom = (op == nk::OP_PHYSDERIV || op == nk::OP_IPDERIV) ? g->d_factor : g->d_metric;
+        if (!a.geom && g->nelem > 0)
+            return fail(NK_ERR_INVALID_ARG, std::string(name) + ": this geometry was uploaded without the stream the operator reads "
+                                                                "(NK_GEOM_METRIC / NK_GEOM_FACTORS)");
     }
     a.lambda = lambda;
     a.nelem = nelem;

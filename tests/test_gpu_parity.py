@@ -212,3 +212,31 @@ def test_repeatable_bitwise(nk, shape, P, deformed):
         y = torch.full_like(x, float("nan"))
         nk.helmholtz_apply(basis, geom, 1.5, x, y)
         assert torch.equal(y, y0)
+
+
+def test_geometry_streams(nk):
+    """nk_geom_upload_streams: a metric-only geometry serves Helmholtz (bit-identical to the full upload) and
+    refuses nk_physderiv; a factors-only geometry the other way round."""
+    P = 3
+    el = K.element(o.TET, P)
+    A, J = K.geometry(o.TET, P, 2, True, zhi=1)
+    basis = nk.Basis(o.TET, P)
+    full = nk.Geom(basis, A.cuda(), J.cuda(), True)
+    gm = nk.Geom(basis, A.cuda(), J.cuda(), True, streams=nk.Geom.METRIC)
+    gf = nk.Geom(basis, A.cuda(), J.cuda(), True, streams=nk.Geom.FACTORS)
+    x = wl.coefficients(5, J.shape[0], el.Nm).cuda()
+    y0, y1 = torch.empty_like(x), torch.empty_like(x)
+    nk.helmholtz_apply(basis, full, 2.0, x, y0)
+    nk.helmholtz_apply(basis, gm, 2.0, x, y1)
+    assert torch.equal(y0, y1)
+    u = wl.point_values(6, J.shape[0], el.Nq).cuda()
+    d = [torch.empty_like(u) for _ in range(3)]
+    nk.physderiv(basis, gf, u, d[0], d[1], d[2])
+    ref = o.physderiv(el, A.numpy(), u.cpu().numpy())
+    assert K.op_err("physderiv", torch.stack(d).cpu().numpy(), ref) <= TOL
+    with pytest.raises(nk.NkError) as ei:
+        nk.physderiv(basis, gm, u, d[0], d[1], d[2])
+    assert ei.value.code == 1
+    with pytest.raises(nk.NkError) as ei:
+        nk.helmholtz_apply(basis, gf, 2.0, x, y1)
+    assert ei.value.code == 1
