@@ -346,7 +346,7 @@ def main():
         pass
     hbm_peak = float(peaks.get("hbm_gbs", HBM_FALLBACK_GBS))
     hbm_src = "MEASURED_PEAKS.json hbm_gbs" if "hbm_gbs" in peaks else "fallback of B200_PROFILING.md"
-    fp64_tf, _ = nk.probe_fp64_peak(100)
+    fp64_tf, _ = nk.probe_fp64_peak(400)
     ach_gbs = alg_bytes / (ms_step * 1e-3) / 1e9
     ach_tf = alg_flops / (ms_step * 1e-3) / 1e12
     hbm_frac, fp_frac = ach_gbs / hbm_peak, ach_tf / fp64_tf

@@ -151,7 +151,7 @@ nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g, double la
                                   double* host_out, void* stream);
 
 /* ---- diagnostics ----------------------------------------------------------------------------- */
-/* Register-only DFMA chains on every SM for about `iters` x 4096 FMAs per thread; *tflops receives the
+/* Register-only DFMA chains on every SM for `iters` x 1024 FMAs per thread (8 independent chains); *tflops receives the
  * sustained fp64 rate (2 flop per FMA).  This is the measured FP64 roofline denominator.            */
 nk_status nk_probe_fp64_peak(int iters, double* tflops, double* ms);
 /* number of kernels this library has launched from the calling process so far                      */
