@@ -48,8 +48,9 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
         const char* ev = std::getenv("NK_PREFETCH_PCT");
         pf_pct = ev ? std::atoi(ev) : 12;
     }
-    b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * pf_pct / 100) + 1 : 0x3fffffff;
-    const long long nblocks = (long long)a.grid_groups * (a.nfields > 1 ? a.nfields : 1);
+    b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * T::WPB * pf_pct / 100) + 1 : 0x3fffffff;
+    const long long units = (long long)a.grid_groups * (a.nfields > 1 ? a.nfields : 1);   // (group, field) pairs
+    const long long nblocks = (units + T::WPB - 1) / T::WPB;                               // WPB of them per block in WP mode
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     kern<<<(unsigned)nblocks, T::NT, smem, stream>>>(tabs, st, b);
     return cudaGetLastError();

@@ -67,12 +67,22 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     constexpr int N1 = SP2 ? NM * (NM + 1) / 2 : NM * NM;
     constexpr int NCG = (OP == OP_PHYSDERIV || OP == OP_IPDERIV) ? 10 : 7;
 
+    constexpr bool WP = T::WP;
     extern __shared__ double sm[];
-    double* __restrict__ X = sm;
-    double* __restrict__ Y = sm + (size_t)NQP * E;
-    double* __restrict__ Z = sm + (size_t)2 * NQP * E;
-    const int tid = threadIdx.x;
+    // block-wide variant: thread = (e, slot) over the whole block; WP variant: the same within each warp,
+    // which owns its own X, Y, Z slice and its own group of E elements
+    const int tid = WP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
+    const int wgrp = WP ? (int)(threadIdx.x >> 5) : 0;
+    double* __restrict__ X = sm + (size_t)wgrp * 3 * NQP * E;
+    double* __restrict__ Y = X + (size_t)NQP * E;
+    double* __restrict__ Z = X + (size_t)2 * NQP * E;
     const int e = tid % E, slot = tid / E;
+    const bool active = !WP || tid < E * LS;     // WP: lanes beyond E*Q^2 (27 of 32 at Q = 3, 25 at Q = 5) idle
+#define NK_SYNC()                                   \
+    do {                                            \
+        if constexpr (WP) __syncwarp();             \
+        else __syncthreads();                       \
+    } while (0)
 #define GIDX(i, j, k) (((i) + LQ * ((j) + Q * (k))) * E + e)
 // partial transforms T1[l][k] (after the r-sum) and T2[p][j][k] (after the q-sum): the k-stride LQ is odd
 // when E < 16, so that threads on consecutive lines l or j fall into different banks
@@ -81,7 +91,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
 
     // simplex stages: warp-uniform roles (see nk_stage_sx.inc)
     constexpr int SPW = T::SPW;
-    const int warp = tid >> 5, sub = (tid & 31) / E;
+    const int warp = (int)(threadIdx.x >> 5), sub = (int)(threadIdx.x & 31) / E;
     (void)warp; (void)sub; (void)st;
 
     // one group per block (grid = ngroups).  NOT a persistent loop: ptxas hoists the constant-bank matrix
@@ -89,13 +99,17 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     // spills per thread and a third of the issue slots lost).
     {
         constexpr bool FIELDS = (OPX == OP_HELMF);
-        const int fld = (FIELDS && a.nfields > 1) ? (int)(blockIdx.x % a.nfields) : 0;
-        const int g = a.g0 + ((FIELDS && a.nfields > 1) ? (int)(blockIdx.x / a.nfields) : (int)blockIdx.x);
+        const long long unit = WP ? (long long)blockIdx.x * T::WPB + wgrp : (long long)blockIdx.x;   // group x field
+        const int fld = (FIELDS && a.nfields > 1) ? (int)(unit % a.nfields) : 0;
+        const int g = a.g0 + ((FIELDS && a.nfields > 1) ? (int)(unit / a.nfields) : (int)unit);
+        if constexpr (WP) {
+            if (g >= a.g0 + a.grid_groups) return;      // surplus warps of the last block (no block barrier in WP mode)
+        }
         // field pointers are re-read from the parameter bank where they are used (no registers held across stages)
 #define NK_FIN0 (FIELDS ? a.fin[fld] : a.in[0])
 #define NK_FOUT0 (FIELDS ? a.fout[fld] : a.out[0])
         const long long elem = (long long)g * E + e;
-        const bool valid = elem < a.nelem;
+        const bool valid = active && elem < a.nelem;
         const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
         (void)geo;
         if constexpr (DEF) {
@@ -110,13 +124,13 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             // the same for the next group's input fields (element-major, contiguous per group)
             constexpr int NIN = IN_COEFF ? NMODES : NQ;
             const int gn = g + a.pf_dist;
-            if (gn < a.ngroups && tid == 32) {
+            if (gn < a.ngroups && tid == (WP ? 0 : 32)) {
                 const double* base = IN_COEFF ? NK_FIN0 : a.in[0];
                 if (base && (reinterpret_cast<size_t>(base) & 15) == 0) {
                     const long long e0 = (long long)gn * E;
                     const long long cnt = (a.nelem - e0 < E) ? (a.nelem - e0) : E;
                     const unsigned bytes = (unsigned)(cnt * NIN * sizeof(double)) & ~15u;
-                    if (bytes) l2_prefetch(base + e0 * NIN, bytes);
+                    if (bytes && (reinterpret_cast<size_t>(base + e0 * NIN) & 15) == 0) l2_prefetch(base + e0 * NIN, bytes);
                 }
             }
         }
@@ -127,7 +141,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             // LDGSTS (cp.async): every trip in flight at once, no registers held, zero-fill for the ragged tail
             NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : NK_FIN0, valid);
             cp_async_wait_all();
-            __syncthreads();
+            NK_SYNC();
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
             if constexpr (!SP1) {
                 NK_FOR(l, NM * NM) {
@@ -144,7 +158,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
 #include "nk_stage_sx.inc"
 #undef NK_SX_STAGE
             }
-            __syncthreads();
+            NK_SYNC();
             // a2/S2: sum over q:  T1 -> T2[p][j][k] in X
             if constexpr (!SP2) {
                 NK_FOR(l, NM * Q) {
@@ -162,7 +176,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
 #include "nk_stage_sx.inc"
 #undef NK_SX_STAGE
             }
-            __syncthreads();
+            NK_SYNC();
 #include "nk_stage_s3.inc"
         } else {
 #include "nk_stage_physin.inc"
@@ -172,6 +186,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     }
 #undef NK_FIN0
 #undef NK_FOUT0
+#undef NK_SYNC
 #undef GIDX
 #undef T1IDX
 #undef T2IDX

@@ -44,13 +44,28 @@ __host__ __device__ constexpr int k_num_modes(int shape, int nm)
 // Values from the round-1 sweeps on B200 (profiles/r1_notes.md): deformed (HBM-bound) kernels want small
 // blocks (about 150-200 threads) at up to 96 registers, many of them per SM; affine (issue / shared-memory
 // bound) kernels want 72 registers and as many resident threads as that allows.
+//
+// WP ("warp-private" elements; the low-order variant, cf. the paper's threading over elements): at
+// Q <= 5 all Q^2 lines of 32/Q^2 elements fit ONE warp.  Each warp then owns its elements and its own slice
+// of shared memory, and the stages are separated by __syncwarp() instead of block barriers, which dominate the
+// run time when a stage is only 9..25 short lines.  Hexes only.  MEASURED SLOWER on B200 and therefore OFF by
+// default (build with -DNK_TUNE_WP=1 to try it): config 4 mass + Laplacian P1 22.0 vs 30.8, P2 37.4 vs 45.7,
+// P3 36.7 vs 40.5 GDoF/s -- the block barriers are not what limits the low orders; the idle lanes (27 or 25 of
+// 32) and the bank conflicts of a 2-3 element interleave cost more than the barriers save.
 template <int SHAPE, int P, int DEF>
 struct Tune {
     static constexpr int Q = P + 2;
-#if defined(NK_TUNE_E)
-    static constexpr int E = NK_TUNE_E;
+#if defined(NK_TUNE_WP)
+    static constexpr bool WP = (NK_TUNE_WP != 0) && SHAPE == K_HEX && Q <= 5;
 #else
-    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : 4)
+    static constexpr bool WP = false;
+#endif
+    static constexpr int WPB = WP ? 8 : 1;          // warps (= independent groups) per block in WP mode
+#if defined(NK_TUNE_E)
+    static constexpr int E = WP ? 32 / (Q * Q) : NK_TUNE_E;
+#else
+    static constexpr int E = WP ? 32 / (Q * Q)
+                             : DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : 4)
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
@@ -77,8 +92,8 @@ struct Tune {
     // used once (nothing for the compiler to hoist and spill)
     static constexpr int LS = SHAPE == K_HEX ? Q * Q : cdiv((Q * Q > LS_min ? Q * Q : LS_min), SPW) * SPW;
 #endif
-    static constexpr int NT = E * LS;
-    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
+    static constexpr int NT = WP ? 32 * WPB : E * LS;
+    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double) * WPB;
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
@@ -162,8 +177,8 @@ __device__ __forceinline__ void static_switch(int v, F&& f)
 // constant so that single-trip stages are straight-line code.
 // NK_FORU: the same, fully unrolled (global loads/stores: all trips in flight at once)
 #define NK_FORU(l, N) \
-    _Pragma("unroll") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (l < (N))
+    _Pragma("unroll") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (active && l < (N))
 #define NK_FOR(l, N) \
-    _Pragma("unroll 1") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (l < (N))
+    _Pragma("unroll 1") for (int l = slot, l##_t = 0; l##_t < ((N) + LS - 1) / LS; ++l##_t, l += LS) if (active && l < (N))
 
 } // namespace nk
