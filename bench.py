@@ -68,6 +68,8 @@ def algorithmic(shape, P, deformed, op="helmholtz"):
         bwd = 2 * (Q * Nm + Q * Q * nm * nm + nm * Q ** 3)
         chain = 4
     if op == "mass":
+        if shape == 0 and not deformed:      # affine hex: three nm x nm contractions in coefficient space
+            return 16 * Nm + 8, 6 * nm ** 4 + Nm
         return 16 * Nm + 8 * (Nq if deformed else 1), 2 * bwd + Nq
     return 16 * Nm + 56 * (Nq if deformed else 1), 2 * bwd + 12 * Q ** 4 + (17 + 2 * chain) * Nq
 

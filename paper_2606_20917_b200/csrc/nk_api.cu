@@ -106,12 +106,19 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     b->inst = get();
     const nk::HostTables& t = b->t;
     const int nm = t.nm;
-    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
+    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], M1[3][nm*nm], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
     std::vector<double>& f = b->tabs_flat;
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
     for (int d = 0; d < 3; ++d)
         for (int p = 0; p < nm; ++p)
             for (int i = 0; i < Q; ++i) f.push_back(t.psi[0][i * nm + p]); // BaT
+    for (int d = 0; d < 3; ++d) // M1 = Ba^T diag(w) Ba with the GLL weights of direction d (hex: all alike)
+        for (int pp = 0; pp < nm; ++pp)
+            for (int p = 0; p < nm; ++p) {
+                double m = 0.0;
+                for (int i = 0; i < Q; ++i) m += t.psi[0][i * nm + pp] * t.w[d][i] * t.psi[0][i * nm + p];
+                f.push_back(m);
+            }
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.D[d].begin(), t.D[d].end());
     for (int d = 0; d < 3; ++d)
         for (int r = 0; r < Q; ++r)
@@ -396,7 +403,7 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     }
     nk_status st = ensure_device();
     if (st != NK_OK) return st;
-    const int E = b->inst->E[(g && g->deformed) ? 1 : 0];
+    const int E = (op == nk::OP_MASS && g && !g->deformed) ? b->inst->E_mass_affine : b->inst->E[(g && g->deformed) ? 1 : 0];
     nk::KArgs a;
     a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
     a.out[0] = out0; a.out[1] = out1; a.out[2] = out2;

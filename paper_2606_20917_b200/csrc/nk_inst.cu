@@ -16,7 +16,7 @@ namespace nk {
 template <int SHAPE, int P, int DEF, int OP>
 static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const KArgs& a, int num_sms, cudaStream_t stream)
 {
-    using T = Tune<SHAPE, P, DEF>;
+    using T = TuneOp<SHAPE, P, DEF, OP>;
     static int blocks_per_sm = 0;
     DenseTabs<P + 1, P + 2> tabs;
     std::memcpy(&tabs, tabs_flat, sizeof(tabs));
@@ -72,6 +72,7 @@ extern "C" const nk::InstInfo* NK_INST_NAME(NK_SHAPE, NK_P)()
     using T0 = nk::Tune<NK_SHAPE, NK_P, 0>;
     using T1 = nk::Tune<NK_SHAPE, NK_P, 1>;
     static const nk::InstInfo info = {NK_SHAPE, NK_P, NK_P + 2, {T0::E, T1::E}, {T0::NT, T1::NT}, {T0::MINB, T1::MINB},
-                                      {T0::smem_grid, T1::smem_grid}, {NK_ROW(0), NK_ROW(1)}};
+                                      {T0::smem_grid, T1::smem_grid}, {NK_ROW(0), NK_ROW(1)},
+                                      nk::TuneOp<NK_SHAPE, NK_P, 0, nk::OP_MASS>::E};
     return &info;
 }

@@ -50,11 +50,11 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, 
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
 template <int SHAPE, int P, int DEF, int OPX>
-__global__ void __launch_bounds__(Tune<SHAPE, P, DEF>::NT, Tune<SHAPE, P, DEF>::MINB)
+__global__ void __launch_bounds__(TuneOp<SHAPE, P, DEF, OPX>::NT, TuneOp<SHAPE, P, DEF, OPX>::MINB)
 nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
           const __grid_constant__ typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st, const __grid_constant__ KArgs a)
 {
-    using T = Tune<SHAPE, P, DEF>;
+    using T = TuneOp<SHAPE, P, DEF, OPX>;
     constexpr int OP = (OPX == OP_HELMF) ? OP_HELM : OPX;
     constexpr int NM = P + 1, Q = P + 2, E = T::E, LS = T::LS, LQ = T::LQ;
     constexpr int NQ = Q * Q * Q, NQP = T::NQP, NMODES = k_num_modes(SHAPE, NM);
@@ -66,6 +66,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     constexpr bool CHAIN = (SHAPE != K_HEX) && !DEF; // deformed simplices: chain folded at upload
     constexpr int N1 = SP2 ? NM * (NM + 1) / 2 : NM * NM;
     constexpr int NCG = (OP == OP_PHYSDERIV || OP == OP_IPDERIV) ? 10 : 7;
+    constexpr bool MASS_KRON = T::MASS_KRON;           // nk_stage_masskron.inc
+    constexpr int EG = Tune<SHAPE, P, DEF>::E;         // interleave width of the geometry stream
 
     constexpr bool WP = T::WP;
     extern __shared__ double sm[];
@@ -74,8 +76,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     const int tid = WP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
     const int wgrp = WP ? (int)(threadIdx.x >> 5) : 0;
     double* __restrict__ X = sm + (size_t)wgrp * 3 * NQP * E;
-    double* __restrict__ Y = X + (size_t)NQP * E;
-    double* __restrict__ Z = X + (size_t)2 * NQP * E;
+    double* __restrict__ Y = X + (size_t)(T::MASS_KRON ? 0 : 1) * NQP * E;   // the coefficient-space mass kernel
+    double* __restrict__ Z = X + (size_t)(T::MASS_KRON ? 1 : 2) * NQP * E;   // ping-pongs between two arrays
     const int e = tid % E, slot = tid / E;
     const bool active = !WP || tid < E * LS;     // WP: lanes beyond E*Q^2 (27 of 32 at Q = 3, 25 at Q = 5) idle
 #define NK_SYNC()                                   \
@@ -111,7 +113,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
         const long long elem = (long long)g * E + e;
         const bool valid = active && elem < a.nelem;
         const double* __restrict__ geo = a.geom + (DEF ? ((size_t)g * NCG * NQ) * E : ((size_t)g * NCG) * E) + e;
-        (void)geo;
+        (void)geo; (void)EG;
         if constexpr (DEF) {
             // stream the NEXT group's geometry (contiguous [NCG][NQ][E] doubles) from DRAM into L2 while this
             // group is being computed: the loads of pass C then hit L2 and HBM stays busy during all stages.
@@ -139,9 +141,16 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             // a1: coefficients -> Y as C[m]
             const double* __restrict__ src = NK_FIN0 + elem * NMODES;
             // LDGSTS (cp.async): every trip in flight at once, no registers held, zero-fill for the ragged tail
-            NK_FORU(m, NMODES) cp_async8(&Y[m * E + e], valid ? src + m : NK_FIN0, valid);
+            constexpr int NMP = T::NMP;
+            (void)NMP;
+            NK_FORU(m, NMODES)
+            cp_async8(MASS_KRON ? &Y[(((m / (NM * NM)) * NMP + (m / NM) % NM) * NMP + m % NM) * E + e] : &Y[m * E + e],
+                      valid ? src + m : NK_FIN0, valid);
             cp_async_wait_all();
             NK_SYNC();
+            if constexpr (MASS_KRON) {
+#include "nk_stage_masskron.inc"
+            } else {
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
             if constexpr (!SP1) {
                 NK_FOR(l, NM * NM) {
@@ -178,11 +187,14 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             }
             NK_SYNC();
 #include "nk_stage_s3.inc"
+            } // !MASS_KRON
         } else {
 #include "nk_stage_physin.inc"
         }
+        if constexpr (!MASS_KRON) {
 #include "nk_stage_mid.inc"
 #include "nk_stage_out.inc"
+        }
     }
 #undef NK_FIN0
 #undef NK_FOUT0

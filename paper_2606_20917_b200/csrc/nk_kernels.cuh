@@ -104,6 +104,30 @@ struct Tune {
 #endif
 };
 
+// Per-operator launch configuration.  Only the affine-hex mass operator in coefficient space
+// (nk_stage_masskron.inc) departs from Tune: it has nm^2 lines of nm entries, no quadrature-point arrays, and
+// is bandwidth-bound, so it takes more elements per block (its own E; the geometry stream keeps Tune's E).
+template <int SHAPE, int P, int DEF, int OPX>
+struct TuneOp : Tune<SHAPE, P, DEF> {
+    using B = Tune<SHAPE, P, DEF>;
+    static constexpr bool MASS_KRON = (OPX == OP_MASS && SHAPE == K_HEX && !DEF && !B::WP);
+    static constexpr int NM = P + 1;
+#if defined(NK_TUNE_EMASS)
+    static constexpr int EK = NK_TUNE_EMASS;
+#else
+    static constexpr int EK = NM <= 2 ? 16 : NM <= 3 ? 8 : NM <= 5 ? 4 : NM <= 9 ? 2 : 1;   // 64..162 threads per block (B200 sweep)
+#endif
+    static constexpr int E = MASS_KRON ? EK : B::E;
+    static constexpr int LQ = MASS_KRON ? B::Q : B::LQ;   // unused by the mass kernel
+    static constexpr int NMP = (NM % 4 == 0) ? NM + 1 : NM;   // padded stride of the coefficient cube
+    static constexpr int NQP = MASS_KRON ? NMP * NMP * NMP : B::NQP;
+    static constexpr int LS = MASS_KRON ? NM * NM : B::LS;
+    static constexpr int NT = MASS_KRON ? E * LS : B::NT;
+    static constexpr size_t smem_grid = MASS_KRON ? (size_t)2 * NQP * E * sizeof(double) : B::smem_grid;
+    static constexpr int MINB_k = 65536 / (NT * 40) > 16 ? 16 : 65536 / (NT * 40);
+    static constexpr int MINB = MASS_KRON ? (MINB_k < 1 ? 1 : MINB_k) : B::MINB;
+};
+
 // ---- kernel parameters (constant bank) -------------------------------------------------
 template <int NM, int Q>
 struct DenseTabs {
@@ -111,6 +135,7 @@ struct DenseTabs {
     double BaT[3][NM * Q]; // [d][p][i]  transposes: operands of the adjoint passes (Eq. 20).
                            // One copy per use site on purpose: loads of one address would be merged by the
                            // compiler, kept in registers from a forward pass to its adjoint, and spilled.
+    double M1[3][NM * NM]; // [d][p'][p]  Ba^T diag(w) Ba: 1-D mass matrix (hex affine mass, nk_stage_masskron.inc)
     double D[3][Q * Q];  // [d][i][r]  D^(d)[i][r] = h_r'(z_i)   (Eq. 22)
     double DT[3][Q * Q]; // [d][r][i]  transposes
     double w[3][Q];      // 1-D weights (collapse Jacobian folded in, A16)
