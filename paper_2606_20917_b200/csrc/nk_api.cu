@@ -106,19 +106,38 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     b->inst = get();
     const nk::HostTables& t = b->t;
     const int nm = t.nm;
-    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], M1[3][nm*nm], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
+    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], KM[3][4][nm*nm], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
     std::vector<double>& f = b->tabs_flat;
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
     for (int d = 0; d < 3; ++d)
         for (int p = 0; p < nm; ++p)
             for (int i = 0; i < Q; ++i) f.push_back(t.psi[0][i * nm + p]); // BaT
-    for (int d = 0; d < 3; ++d) // M1 = Ba^T diag(w) Ba with the GLL weights of direction d (hex: all alike)
-        for (int pp = 0; pp < nm; ++pp)
-            for (int p = 0; p < nm; ++p) {
-                double m = 0.0;
-                for (int i = 0; i < Q; ++i) m += t.psi[0][i * nm + pp] * t.w[d][i] * t.psi[0][i * nm + p];
-                f.push_back(m);
+    {   // KM[stage][which]: stage 0 acts on index r (direction 3), 1 on q (direction 2), 2 on p (direction 1);
+        // which = M, K, C, C^T built from psi^a, D and w of that direction (used on hexes only: all alike there)
+        std::vector<double> DB((size_t)Q * nm);
+        for (int st = 0; st < 3; ++st) {
+            const int dir = 2 - st;
+            for (int i = 0; i < Q; ++i)
+                for (int p = 0; p < nm; ++p) {
+                    double s = 0.0;
+                    for (int r = 0; r < Q; ++r) s += t.D[dir][i * Q + r] * t.psi[0][r * nm + p];
+                    DB[(size_t)i * nm + p] = s;
+                }
+            for (int which = 0; which < 4; ++which) {
+                if (shape != NK_HEX) { f.push_back(0.0); continue; }   // DenseTabs<.,.,false>: one dummy entry
+                for (int pp = 0; pp < nm; ++pp)
+                    for (int p = 0; p < nm; ++p) {
+                        double m = 0.0;
+                        for (int i = 0; i < Q; ++i) {
+                            const double w = t.w[dir][i], b1 = t.psi[0][i * nm + pp], b0 = t.psi[0][i * nm + p];
+                            const double d1 = DB[(size_t)i * nm + pp], d0 = DB[(size_t)i * nm + p];
+                            m += w * (which == 0 ? b1 * b0 : which == 1 ? d1 * d0 : which == 2 ? b1 * d0 : d1 * b0);
+                        }
+                        f.push_back(m);
+                    }
             }
+        }
+    }
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.D[d].begin(), t.D[d].end());
     for (int d = 0; d < 3; ++d)
         for (int r = 0; r < Q; ++r)
@@ -403,7 +422,7 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     }
     nk_status st = ensure_device();
     if (st != NK_OK) return st;
-    const int E = (op == nk::OP_MASS && g && !g->deformed) ? b->inst->E_mass_affine : b->inst->E[(g && g->deformed) ? 1 : 0];
+    const int E = (g && g->deformed) ? b->inst->E[1] : b->inst->E_op_affine[op];
     nk::KArgs a;
     a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
     a.out[0] = out0; a.out[1] = out1; a.out[2] = out2;
@@ -516,16 +535,18 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
         }
         if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: stream / event creation");
     }
-    const int64_t per = (g->ngroups + nk_geom::kChunks - 1) / nk_geom::kChunks;
+    const int Eop = g->deformed ? b->inst->E[1] : b->inst->E_op_affine[nk::OP_HELM];   // groups of the kernel, not of the stream
+    const int64_t ngroups_op = (g->nelem + Eop - 1) / Eop;
+    const int64_t per = (ngroups_op + nk_geom::kChunks - 1) / nk_geom::kChunks;
     const size_t elem_bytes = (size_t)b->t.Nm * sizeof(double);
     e = cudaEventRecord(g->ev_start, s);                  // order after the caller's earlier work on `stream`
     if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_in, g->ev_start, 0);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_out, g->ev_start, 0);
     if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: pipeline start");
     for (int c = 0; c < nk_geom::kChunks; ++c) {
-        const int64_t g0 = c * per, g1 = std::min<int64_t>(g->ngroups, g0 + per);
+        const int64_t g0 = c * per, g1 = std::min<int64_t>(ngroups_op, g0 + per);
         if (g0 >= g1) break;
-        const int64_t e0 = g0 * g->E, e1 = std::min<int64_t>(g->nelem, g1 * g->E);
+        const int64_t e0 = g0 * Eop, e1 = std::min<int64_t>(g->nelem, g1 * Eop);
         const size_t off = (size_t)e0 * b->t.Nm, nb = (size_t)(e1 - e0) * elem_bytes;
         e = cudaMemcpyAsync(g->d_stage_in + off, host_in + off, nb, cudaMemcpyHostToDevice, g->s_in);
         if (e == cudaSuccess) e = cudaEventRecord(g->ev_in[c], g->s_in);

@@ -18,7 +18,7 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
 {
     using T = TuneOp<SHAPE, P, DEF, OP>;
     static int blocks_per_sm = 0;
-    DenseTabs<P + 1, P + 2> tabs;
+    DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs;
     std::memcpy(&tabs, tabs_flat, sizeof(tabs));
     typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st;
     if (SHAPE != K_HEX)
@@ -73,6 +73,10 @@ extern "C" const nk::InstInfo* NK_INST_NAME(NK_SHAPE, NK_P)()
     using T1 = nk::Tune<NK_SHAPE, NK_P, 1>;
     static const nk::InstInfo info = {NK_SHAPE, NK_P, NK_P + 2, {T0::E, T1::E}, {T0::NT, T1::NT}, {T0::MINB, T1::MINB},
                                       {T0::smem_grid, T1::smem_grid}, {NK_ROW(0), NK_ROW(1)},
-                                      nk::TuneOp<NK_SHAPE, NK_P, 0, nk::OP_MASS>::E};
+                                      {nk::TuneOp<NK_SHAPE, NK_P, 0, 0>::E, nk::TuneOp<NK_SHAPE, NK_P, 0, 1>::E,
+                                       nk::TuneOp<NK_SHAPE, NK_P, 0, 2>::E, nk::TuneOp<NK_SHAPE, NK_P, 0, 3>::E,
+                                       nk::TuneOp<NK_SHAPE, NK_P, 0, 4>::E, nk::TuneOp<NK_SHAPE, NK_P, 0, 5>::E,
+                                       nk::TuneOp<NK_SHAPE, NK_P, 0, 6>::E, nk::TuneOp<NK_SHAPE, NK_P, 0, 7>::E}};
+    static_assert(nk::OP_COUNT == 8, "update E_op_affine");
     return &info;
 }

@@ -51,7 +51,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 
 template <int SHAPE, int P, int DEF, int OPX>
 __global__ void __launch_bounds__(TuneOp<SHAPE, P, DEF, OPX>::NT, TuneOp<SHAPE, P, DEF, OPX>::MINB)
-nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
+nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
           const __grid_constant__ typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st, const __grid_constant__ KArgs a)
 {
     using T = TuneOp<SHAPE, P, DEF, OPX>;
@@ -67,6 +67,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     constexpr int N1 = SP2 ? NM * (NM + 1) / 2 : NM * NM;
     constexpr int NCG = (OP == OP_PHYSDERIV || OP == OP_IPDERIV) ? 10 : 7;
     constexpr bool MASS_KRON = T::MASS_KRON;           // nk_stage_masskron.inc
+    constexpr bool LAP_KRON = T::LAP_KRON;             // nk_stage_lapkron.inc
+    constexpr bool KRON = T::KRON;
     constexpr int EG = Tune<SHAPE, P, DEF>::E;         // interleave width of the geometry stream
 
     constexpr bool WP = T::WP;
@@ -75,9 +77,11 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
     // which owns its own X, Y, Z slice and its own group of E elements
     const int tid = WP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
     const int wgrp = WP ? (int)(threadIdx.x >> 5) : 0;
-    double* __restrict__ X = sm + (size_t)wgrp * 3 * NQP * E;
-    double* __restrict__ Y = X + (size_t)(T::MASS_KRON ? 0 : 1) * NQP * E;   // the coefficient-space mass kernel
-    double* __restrict__ Z = X + (size_t)(T::MASS_KRON ? 1 : 2) * NQP * E;   // ping-pongs between two arrays
+    // general path: X, Y, Z; coefficient-space kernels: Y, Z, X(, fourth array) in that order (see their .inc)
+    double* __restrict__ S0 = sm + (size_t)wgrp * 3 * NQP * E;
+    double* __restrict__ X = S0 + (size_t)(T::KRON ? 2 : 0) * NQP * E;
+    double* __restrict__ Y = S0 + (size_t)(T::KRON ? 0 : 1) * NQP * E;
+    double* __restrict__ Z = S0 + (size_t)(T::KRON ? 1 : 2) * NQP * E;
     const int e = tid % E, slot = tid / E;
     const bool active = !WP || tid < E * LS;     // WP: lanes beyond E*Q^2 (27 of 32 at Q = 3, 25 at Q = 5) idle
 #define NK_SYNC()                                   \
@@ -144,12 +148,14 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             constexpr int NMP = T::NMP;
             (void)NMP;
             NK_FORU(m, NMODES)
-            cp_async8(MASS_KRON ? &Y[(((m / (NM * NM)) * NMP + (m / NM) % NM) * NMP + m % NM) * E + e] : &Y[m * E + e],
+            cp_async8(KRON ? &Y[(((m / (NM * NM)) * NMP + (m / NM) % NM) * NMP + m % NM) * E + e] : &Y[m * E + e],
                       valid ? src + m : NK_FIN0, valid);
             cp_async_wait_all();
             NK_SYNC();
             if constexpr (MASS_KRON) {
 #include "nk_stage_masskron.inc"
+            } else if constexpr (LAP_KRON) {
+#include "nk_stage_lapkron.inc"
             } else {
             // a2/S1: sum over r  (Eq. 16 innermost / Eq. 17 innermost):  C -> T1[l][k] in Z
             if constexpr (!SP1) {
@@ -187,11 +193,11 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2> tabs,
             }
             NK_SYNC();
 #include "nk_stage_s3.inc"
-            } // !MASS_KRON
+            } // !KRON
         } else {
 #include "nk_stage_physin.inc"
         }
-        if constexpr (!MASS_KRON) {
+        if constexpr (!KRON) {
 #include "nk_stage_mid.inc"
 #include "nk_stage_out.inc"
         }

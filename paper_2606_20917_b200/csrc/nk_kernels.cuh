@@ -110,32 +110,55 @@ struct Tune {
 template <int SHAPE, int P, int DEF, int OPX>
 struct TuneOp : Tune<SHAPE, P, DEF> {
     using B = Tune<SHAPE, P, DEF>;
-    static constexpr bool MASS_KRON = (OPX == OP_MASS && SHAPE == K_HEX && !DEF && !B::WP);
+    static constexpr bool AFF_HEX = (SHAPE == K_HEX && !DEF && !B::WP);
+    static constexpr bool MASS_KRON = AFF_HEX && OPX == OP_MASS;                                   // nk_stage_masskron.inc
+#if defined(NK_NO_LAPKRON)
+    static constexpr bool LAP_KRON = false;
+#else
+    // nk_stage_lapkron.inc; up to P = 7: beyond, its stage 2 (4 nm inputs + 9 accumulators in registers) spills and the
+    // quadrature-grid path is faster (B200: P8 49 vs 59 GDoF/s)
+    static constexpr bool LAP_KRON = AFF_HEX && (P + 1) <= 8 && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
+#endif
+    static constexpr bool KRON = MASS_KRON || LAP_KRON;
     static constexpr int NM = P + 1;
 #if defined(NK_TUNE_EMASS)
     static constexpr int EK = NK_TUNE_EMASS;
 #else
     static constexpr int EK = NM <= 2 ? 16 : NM <= 3 ? 8 : NM <= 5 ? 4 : NM <= 9 ? 2 : 1;   // 64..162 threads per block (B200 sweep)
 #endif
-    static constexpr int E = MASS_KRON ? EK : B::E;
-    static constexpr int LQ = MASS_KRON ? B::Q : B::LQ;   // unused by the mass kernel
+#if defined(NK_TUNE_ELAP)
+    static constexpr int EL = NK_TUNE_ELAP;
+#else
+    static constexpr int EL = NM <= 2 ? 16 : NM <= 3 ? 8 : NM <= 5 ? 4 : NM <= 6 ? 2 : 1;   // B200 sweep (r1_notes.md)
+#endif
+    static constexpr int E = MASS_KRON ? EK : LAP_KRON ? EL : B::E;
+    static constexpr int LQ = KRON ? B::Q : B::LQ;        // unused by the coefficient-space kernels
     static constexpr int NMP = (NM % 4 == 0) ? NM + 1 : NM;   // padded stride of the coefficient cube
-    static constexpr int NQP = MASS_KRON ? NMP * NMP * NMP : B::NQP;
-    static constexpr int LS = MASS_KRON ? NM * NM : B::LS;
-    static constexpr int NT = MASS_KRON ? E * LS : B::NT;
-    static constexpr size_t smem_grid = MASS_KRON ? (size_t)2 * NQP * E * sizeof(double) : B::smem_grid;
-    static constexpr int MINB_k = 65536 / (NT * 40) > 16 ? 16 : 65536 / (NT * 40);
-    static constexpr int MINB = MASS_KRON ? (MINB_k < 1 ? 1 : MINB_k) : B::MINB;
+    static constexpr int NQP = KRON ? NMP * NMP * NMP : B::NQP;
+    static constexpr int NARR = MASS_KRON ? 2 : LAP_KRON ? 4 : 3;
+    static constexpr int LS = KRON ? NM * NM : B::LS;
+    static constexpr int NT = KRON ? E * LS : B::NT;
+    static constexpr size_t smem_grid = KRON ? (size_t)NARR * NQP * E * sizeof(double) : B::smem_grid;
+#if defined(NK_TUNE_REGSK)
+    static constexpr int REGSK = NK_TUNE_REGSK;
+#else
+    static constexpr int REGSK = MASS_KRON ? 40 : NM <= 2 ? 64 : NM <= 4 ? 96 : 128;
+#endif
+    static constexpr int MINB_k = 65536 / (NT * REGSK) > 16 ? 16 : 65536 / (NT * REGSK);
+    static constexpr int MINB = KRON ? (MINB_k < 1 ? 1 : MINB_k) : B::MINB;
 };
 
 // ---- kernel parameters (constant bank) -------------------------------------------------
-template <int NM, int Q>
+template <int NM, int Q, bool HEXK = true>
 struct DenseTabs {
     double Ba[3][Q * NM];  // [d][i][p]  psi^a_p at the GLL points, one copy per direction that uses it
     double BaT[3][NM * Q]; // [d][p][i]  transposes: operands of the adjoint passes (Eq. 20).
                            // One copy per use site on purpose: loads of one address would be merged by the
                            // compiler, kept in registers from a forward pass to its adjoint, and spilled.
-    double M1[3][NM * NM]; // [d][p'][p]  Ba^T diag(w) Ba: 1-D mass matrix (hex affine mass, nk_stage_masskron.inc)
+    // 1-D matrices of the coefficient-space (Kronecker) form of the affine hex operators, [stage][which][p'][p]:
+    // which = 0: M = Ba^T w Ba, 1: K = (D Ba)^T w (D Ba), 2: C = Ba^T w (D Ba), 3: C^T; stage 0 acts on index r,
+    // 1 on q, 2 on p (one copy per stage: see Ba).  nk_stage_masskron.inc, nk_stage_lapkron.inc
+    double KM[3][4][HEXK ? NM * NM : 1];   // hexes only (one dummy entry each on simplices: parameter space)
     double D[3][Q * Q];  // [d][i][r]  D^(d)[i][r] = h_r'(z_i)   (Eq. 22)
     double DT[3][Q * Q]; // [d][r][i]  transposes
     double w[3][Q];      // 1-D weights (collapse Jacobian folded in, A16)

@@ -14,7 +14,7 @@ struct InstInfo {
     int E[2], threads[2], blocks_per_sm_hint[2]; // [deformed]
     size_t smem_grid[2];
     LaunchFn fn[2][OP_COUNT]; // [deformed][op]
-    int E_mass_affine;        // elements per block of the affine mass kernel (TuneOp)
+    int E_op_affine[OP_COUNT]; // elements per block of each AFFINE kernel (TuneOp; the geometry stream keeps E[0])
 };
 
 } // namespace nk
