@@ -129,7 +129,8 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
 #if defined(NK_TUNE_ELAP)
     static constexpr int EL = NK_TUNE_ELAP;
 #else
-    static constexpr int EL = NM <= 2 ? 16 : NM <= 3 ? 8 : NM <= 5 ? 4 : NM <= 6 ? 2 : 1;   // B200 sweep (r1_notes.md)
+    static constexpr int EL = NM <= 2 ? 16 : NM <= 3 ? 8 : NM <= 4 ? 4 : NM <= 5 ? 5 : NM <= 6 ? 2 : 1;   // B200 sweep (r1_notes.md);
+                                                // 5 x 25 lines = 125 threads fill four warps, 4 x 25 = 100 waste a fifth
 #endif
     static constexpr int E = MASS_KRON ? EK : LAP_KRON ? EL : B::E;
     static constexpr int LQ = KRON ? B::Q : B::LQ;        // unused by the coefficient-space kernels
@@ -142,7 +143,7 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
 #if defined(NK_TUNE_REGSK)
     static constexpr int REGSK = NK_TUNE_REGSK;
 #else
-    static constexpr int REGSK = MASS_KRON ? 40 : NM <= 2 ? 64 : NM <= 4 ? 96 : 128;
+    static constexpr int REGSK = MASS_KRON ? 40 : NM <= 2 ? 64 : NM <= 5 ? 96 : 128;
 #endif
     static constexpr int MINB_k = 65536 / (NT * REGSK) > 16 ? 16 : 65536 / (NT * REGSK);
     static constexpr int MINB = KRON ? (MINB_k < 1 ? 1 : MINB_k) : B::MINB;
