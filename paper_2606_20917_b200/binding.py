@@ -84,10 +84,18 @@ def _dev_ptr(t, allow_none=False):
     return _ptr(t, allow_none)
 
 
+# torch.cuda.current_stream() costs 3 us per call, as much as a small kernel: take the raw handle of torch's
+# current stream directly when this torch has the private accessors (same stream, 0.3 us)
+_raw_stream = getattr(torch._C, "_cuda_getCurrentRawStream", None)
+_raw_device = getattr(torch._C, "_cuda_getDevice", None)
+
+
 def _stream(stream=None):
-    if stream is None:
-        stream = torch.cuda.current_stream()
-    return stream.cuda_stream
+    if stream is not None:
+        return stream.cuda_stream
+    if _raw_stream is not None and _raw_device is not None:
+        return _raw_stream(_raw_device())
+    return torch.cuda.current_stream().cuda_stream
 
 
 class Basis:
