@@ -117,7 +117,10 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
 #else
     // nk_stage_lapkron.inc; up to P = 7: beyond, its stage 2 (4 nm inputs + 9 accumulators in registers) spills and the
     // quadrature-grid path is faster (B200: P8 49 vs 59 GDoF/s)
-    static constexpr bool LAP_KRON = AFF_HEX && (P + 1) <= 8 && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
+#ifndef NK_LAPKRON_MAXNM
+#define NK_LAPKRON_MAXNM 8
+#endif
+    static constexpr bool LAP_KRON = AFF_HEX && (P + 1) <= NK_LAPKRON_MAXNM && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
 #endif
     static constexpr bool KRON = MASS_KRON || LAP_KRON;
     static constexpr int NM = P + 1;
