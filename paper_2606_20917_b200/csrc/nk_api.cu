@@ -106,7 +106,7 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     b->inst = get();
     const nk::HostTables& t = b->t;
     const int nm = t.nm;
-    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], KM[3][4][nm*nm], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[4][Q]
+    // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], KM[3][4][nm*nm], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[7][Q]
     std::vector<double>& f = b->tabs_flat;
     for (int d = 0; d < 3; ++d) f.insert(f.end(), t.psi[0].begin(), t.psi[0].end()); // psi^a at GLL, [i][p]
     for (int d = 0; d < 3; ++d)
@@ -147,6 +147,12 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     for (int i = 0; i < Q; ++i) f.push_back(1.0 + t.z[1][i]);
     for (int i = 0; i < Q; ++i) f.push_back(shape == NK_TET ? 1.0 / (1.0 - t.z[1][i]) : 0.0);
     for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? 1.0 / (1.0 - t.z[2][i]) : 0.0);
+    for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? (1.0 - t.z[2][i]) : 0.0);
+    for (int i = 0; i < Q; ++i) {
+        const double s = shape != NK_HEX ? 1.0 / (1.0 - t.z[2][i]) : 0.0;
+        f.push_back(shape == NK_TET ? t.w[2][i] * s * s : t.w[2][i] * s);
+    }
+    for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? t.w[2][i] / (1.0 - t.z[2][i]) : 0.0);
     // SimplexTabs: b3f, b3a (psi^b at the direction-3 points), b2f, b2a (direction 2; tet only)
     if (shape != NK_HEX) {
         std::vector<double>& x = b->sx_flat;

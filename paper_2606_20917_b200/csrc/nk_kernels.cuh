@@ -166,7 +166,7 @@ struct DenseTabs {
     double D[3][Q * Q];  // [d][i][r]  D^(d)[i][r] = h_r'(z_i)   (Eq. 22)
     double DT[3][Q * Q]; // [d][r][i]  transposes
     double w[3][Q];      // 1-D weights (collapse Jacobian folded in, A16)
-    double aux[4][Q];    // chain helpers (A17): 1+z1, 1+z2, 1/(1-z2), 1/(1-z3)
+    double aux[7][Q];    // chain helpers (A17): 1+z1, 1+z2, 1/(1-z2), s = 1/(1-z3), 1/s, w3 s^2 (tet) or w3 s (prism), w3 s
 };
 
 // pair index of the psi^b tables: row (a,b), a+b <= P  ->  sum_{c<a}(nm-c) + b
