@@ -152,12 +152,16 @@ def test_operator_identities_on_gpu(nk):
         assert K.normwise_err(h, l2 + lam * m2) <= 1e-13
 
 
-def test_helmholtz_host_entry(nk):
+@pytest.mark.parametrize("deformed", [True, False])
+def test_helmholtz_host_entry(nk, deformed):
+    """deformed: quadrature-grid kernel; affine: coefficient-space kernel, whose block size differs from the
+    interleave width of the geometry stream (the chunks of the host pipeline follow the kernel's groups)."""
     P = 4
     el = K.element(o.HEX, P)
-    A, J = K.geometry(o.HEX, P, 3, True)
+    full = K.mesh(o.HEX, 3)[0].shape[0]
+    A, J = K.geometry(o.HEX, P, 3, deformed, take=torch.arange(full - 2))
     basis = nk.Basis(o.HEX, P)
-    geom = nk.Geom(basis, A.cuda(), J.cuda(), True)
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), deformed)
     x = wl.coefficients(21, J.shape[0], el.Nm).pin_memory()
     y = torch.empty_like(x).pin_memory()
     n0 = nk.launch_count()
@@ -167,7 +171,7 @@ def test_helmholtz_host_entry(nk):
     assert K.normwise_err(y.numpy(), ref) <= TOL
 
 
-@pytest.mark.parametrize("shape,deformed", [(o.HEX, True), (o.TET, False), (o.PRISM, True)])
+@pytest.mark.parametrize("shape,deformed", [(o.HEX, True), (o.HEX, False), (o.TET, False), (o.PRISM, True)])
 def test_helmholtz_fields(nk, shape, deformed):
     """nk_helmholtz_apply_fields (multi-field block): each field equals the oracle's Helmholtz of that
     field, and is bit-identical to the single-field call."""
