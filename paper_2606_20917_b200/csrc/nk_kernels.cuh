@@ -97,7 +97,7 @@ struct Tune {
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
-    static constexpr int REGS = DEF ? 96 : Q <= 6 ? 56 : 64;
+    static constexpr int REGS = DEF ? (SHAPE == K_HEX ? 96 : 72) : Q <= 6 ? 56 : 64;
     static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + 2048));
     static constexpr int MINB_reg = 65536 / (NT * REGS);
     static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
