@@ -51,6 +51,8 @@ typedef enum {
     NK_TAB_NODES = 0,   /* z^(dir)[Q]                                              */
     NK_TAB_WEIGHTS = 1, /* w^(dir)[Q], collapse Jacobian folded in (A16)           */
     NK_TAB_DERIV = 2,   /* D^(dir)[Q][Q], D[i][r] = h_r'(z_i) (Eq. 22; A5)  */
+    NK_TAB_KRON = 4,    /* hexes only; dir 0: M = B^T w B, 1: K = (DB)^T w (DB), 2: C = B^T w (DB), each [nm][nm], row =
+                           test mode: the 1-D matrices of the coefficient-space form of the affine operators       */
     NK_TAB_PSI = 3      /* dir 0: psi^a_p(z1_i) as [Q][nm];
                            dir 1: hex/prism psi^a_q(z2_j) as [Q][nm];
                                   tet psi^b_{pq}(z2_j) as [Q][nm(nm+1)/2], column (p,q) = sum_{a<p}(nm-a)+q;

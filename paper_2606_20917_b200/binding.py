@@ -11,7 +11,7 @@ import torch
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.environ.get("NK_LIB") or os.path.join(HERE, "libnk.so")   # NK_LIB: another build of the same library
 HEX, TET, PRISM = 0, 1, 2
-TAB_NODES, TAB_WEIGHTS, TAB_DERIV, TAB_PSI = 0, 1, 2, 3
+TAB_NODES, TAB_WEIGHTS, TAB_DERIV, TAB_PSI, TAB_KRON = 0, 1, 2, 3, 4
 
 if not os.path.exists(LIB_PATH):
     raise ImportError("libnk.so not built (%s): run `python -m paper_2606_20917_b200.build`; "

@@ -69,6 +69,7 @@ struct nk_basis {
     const nk::InstInfo* inst = nullptr;
     std::vector<double> tabs_flat; // DenseTabs<nm,Q> in declaration order
     std::vector<double> sx_flat;   // SimplexTabs in declaration order (simplices only)
+    std::vector<double> kron[3];   // hex: the 1-D matrices M, K, C of the coefficient-space forms (NK_TAB_KRON)
 };
 
 struct nk_geom {
@@ -134,6 +135,7 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
                             m += w * (which == 0 ? b1 * b0 : which == 1 ? d1 * d0 : which == 2 ? b1 * d0 : d1 * b0);
                         }
                         f.push_back(m);
+                        if (st == 2 && which < 3) b->kron[which].push_back(m);
                     }
             }
         }
@@ -187,6 +189,10 @@ extern "C" nk_status nk_basis_get_table(const nk_basis* b, int which, int dir, d
     case NK_TAB_WEIGHTS: v = &b->t.w[dir]; break;
     case NK_TAB_DERIV: v = &b->t.D[dir]; break;
     case NK_TAB_PSI: v = &b->t.psi[dir]; break;
+    case NK_TAB_KRON:
+        if (b->t.shape != nk::HEX) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_table: NK_TAB_KRON exists on hexes only");
+        v = &b->kron[dir];
+        break;
     default: return fail(NK_ERR_INVALID_ARG, "nk_basis_get_table: unknown table");
     }
     if (count) *count = v->size();

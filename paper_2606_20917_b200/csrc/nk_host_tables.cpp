@@ -1,5 +1,5 @@
 // nk_host_tables.cpp -- host precompute (layer B2): nodes, weights, derivative
-// matrices, modified-basis tables and the sparse index arrays of the simplex
+// matrices, modified-basis tables and the row-major psi^b tables of the simplex
 // contractions.  The formulas are deliberately NOT the ones oracle/ uses:
 //   nodes     GLL: Newton on L_N' with Legendre recurrences from Chebyshev-Lobatto
 //             guesses; GRJ: Newton with deflation on P^{alpha,1}_{Q-1}
@@ -229,7 +229,7 @@ bool build_host_tables(int shape, int P, int Q, HostTables& t)
     t.n1 = 0;
     if (shape == HEX) return true;
 
-    // ---- sparse stages of the simplices (Eq. 17 / Eq. 21 with A8) -------------------------
+    // ---- row-major psi^b tables of the triangular stages (Eq. 17 / Eq. 21) -------------------
     t.tab3.assign((size_t)t.npair * Q, 0.0);
     for (int row = 0; row < t.npair; ++row)
         for (int k = 0; k < Q; ++k) t.tab3[(size_t)row * Q + k] = t.psi[2][(size_t)k * t.npair + row];

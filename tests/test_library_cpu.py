@@ -93,3 +93,33 @@ def test_error_codes_and_no_cpu_fallback():
         assert code == 5, nk.lib.nk_last_error()
         with pytest.raises(ValueError):
             nk.bwdtrans(b, x, y)
+
+
+def test_kronecker_matrices_of_the_affine_hex_forms():
+    """M = B^T w B, K = (DB)^T w (DB), C = B^T w (DB) that csrc/nk_stage_masskron.inc and nk_stage_lapkron.inc
+    use: against the exact rational 1-D mass / stiffness matrices of the modified basis at P = 4
+    (tests/golden/modified_basis_P4.txt) and against the oracle's tables at other orders; C + C^T is the
+    boundary term [psi_p psi_q] from -1 to 1 (integration by parts)."""
+    ref = {"M1": np.zeros((5, 5)), "K1": np.zeros((5, 5))}
+    for name, i, j, val in G.records("modified_basis_P4.txt"):
+        ref[name][int(i), int(j)] = ref[name][int(j), int(i)] = G.number(val)
+    b = nk.Basis(o.HEX, 4)
+    M = b.table(nk.TAB_KRON, 0).numpy().reshape(5, 5)
+    Kk = b.table(nk.TAB_KRON, 1).numpy().reshape(5, 5)
+    np.testing.assert_allclose(M, ref["M1"], atol=2e-15)
+    np.testing.assert_allclose(Kk, ref["K1"], atol=2e-14)
+    for P in (1, 3, 6, 10):
+        b = nk.Basis(o.HEX, P)
+        el = o.Element(o.HEX, P, P + 2)
+        nm = P + 1
+        B = np.stack([o.psi_a(p, el.z[0]) for p in range(nm)], axis=1)             # [Q][nm]
+        DB = el.D[0] @ B
+        w = el.w[0]
+        np.testing.assert_allclose(b.table(nk.TAB_KRON, 0).numpy().reshape(nm, nm), B.T @ (w[:, None] * B), atol=1e-14)
+        np.testing.assert_allclose(b.table(nk.TAB_KRON, 1).numpy().reshape(nm, nm), DB.T @ (w[:, None] * DB), atol=1e-12)
+        C = b.table(nk.TAB_KRON, 2).numpy().reshape(nm, nm)
+        np.testing.assert_allclose(C, B.T @ (w[:, None] * DB), atol=1e-13)
+        bnd = np.outer(B[-1], B[-1]) - np.outer(B[0], B[0])                      # psi_p psi_q at +1 minus at -1
+        np.testing.assert_allclose(C + C.T, bnd, atol=1e-13)
+    with pytest.raises(nk.NkError):
+        nk.Basis(o.TET, 3).table(nk.TAB_KRON, 0)
