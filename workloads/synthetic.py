@@ -96,10 +96,26 @@ def prism_mesh(n, zlo=0, zhi=None, device="cpu"):
 # ----------------------------------------------------------------------------
 # geometric factors
 # ----------------------------------------------------------------------------
+def _inv3_det3(M):
+    """Inverse and determinant of a batch of 3x3 matrices [..., 3, 3] by cofactors: elementwise arithmetic only.
+    No library routine (batched LU, GEMM) on purpose: on the GPU those may pick another algorithm from one process
+    to the next, and a full-size parity test then fails on its INPUTS (seen on B200: the first elements of config 2
+    2e-10 away from the host evaluation in one run out of five when the factors went through einsum / linalg)."""
+    a, b, c = M[..., 0, 0], M[..., 0, 1], M[..., 0, 2]
+    d, e, f = M[..., 1, 0], M[..., 1, 1], M[..., 1, 2]
+    g, h, i = M[..., 2, 0], M[..., 2, 1], M[..., 2, 2]
+    c00, c01, c02 = e * i - f * h, f * g - d * i, d * h - e * g
+    det = a * c00 + b * c01 + c * c02
+    adj = torch.stack([torch.stack([c00, c * h - b * i, b * f - c * e], dim=-1),
+                       torch.stack([c01, a * i - c * g, c * d - a * f], dim=-1),
+                       torch.stack([c02, b * g - a * h, a * e - b * d], dim=-1)], dim=-2)
+    return adj / det[..., None, None], det
+
+
 def affine_factors(v0, E):
     """dxi_dx [ne][1][3][3] = (E/2)^-1, detJ [ne][1] = |det(E/2)|."""
-    Jm = 0.5 * E
-    return torch.linalg.inv(Jm)[:, None].contiguous(), torch.linalg.det(Jm).abs()[:, None].contiguous()
+    inv, det = _inv3_det3(0.5 * E)
+    return inv[:, None].contiguous(), det.abs()[:, None].contiguous()
 
 
 def sinusoidal_factors(v0, E, xi, amp=0.05, chunk=4096):
@@ -117,16 +133,16 @@ def sinusoidal_factors(v0, E, xi, amp=0.05, chunk=4096):
     for s0 in range(0, ne, chunk):
         sl = slice(s0, min(ne, s0 + chunk))
         Jm = 0.5 * E[sl]
-        Ainv = torch.linalg.inv(Jm)                                  # [c,3,3]
-        x = v0[sl, None, :] + torch.einsum("cab,nb->cna", Jm, xi + 1.0)
+        Ainv, detA = _inv3_det3(Jm)                                  # [c,3,3], [c]
+        x = v0[sl, None, :] + (Jm[:, None, :, :] * (xi + 1.0)[None, :, None, :]).sum(-1)      # [c,n,3]
         sn, cs = torch.sin(tp * x), torch.cos(tp * x)
         g = tp * torch.stack([cs[..., 0] * sn[..., 1] * sn[..., 2],
                               sn[..., 0] * cs[..., 1] * sn[..., 2],
                               sn[..., 0] * sn[..., 1] * cs[..., 2]], dim=-1)   # grad s
         detF = 1.0 + amp * g.sum(-1)
         Finv = torch.eye(3, dtype=F64, device=dev) - amp * ones[:, None] * g[..., None, :] / detF[..., None, None]
-        A[sl] = torch.einsum("cjk,cnki->cnji", Ainv, Finv)
-        J[sl] = torch.linalg.det(Jm).abs()[:, None] * detF
+        A[sl] = (Ainv[:, None, :, :, None] * Finv[:, :, None, :, :]).sum(-2)                  # A_jk Finv_ki
+        J[sl] = detA.abs()[:, None] * detF
     return A, J
 
 
