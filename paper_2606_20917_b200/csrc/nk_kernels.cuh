@@ -149,7 +149,14 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
     static constexpr int REGSK = MASS_KRON ? 40 : NM <= 2 ? 64 : NM <= 5 ? 96 : 128;
 #endif
     static constexpr int MINB_k = 65536 / (NT * REGSK) > 16 ? 16 : 65536 / (NT * REGSK);
-    static constexpr int MINB = KRON ? (MINB_k < 1 ? 1 : MINB_k) : B::MINB;
+    // affine tet P4 Laplacian / Helmholtz: 48 registers = 8 blocks of 160 threads per SM (24 B of spills) instead of 7 at
+    // 56: 20.67 against 20.43 GDoF/s (r1_notes.md 16); the other operators of that block spill more and keep 56
+#if defined(NK_TUNE_MINB)
+    static constexpr bool TET48 = false;
+#else
+    static constexpr bool TET48 = SHAPE == K_TET && !DEF && P == 4 && B::E == 4 && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
+#endif
+    static constexpr int MINB = KRON ? (MINB_k < 1 ? 1 : MINB_k) : TET48 ? 8 : B::MINB;
 };
 
 // ---- kernel parameters (constant bank) -------------------------------------------------
