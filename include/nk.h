@@ -152,6 +152,24 @@ nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double 
 nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g, double lambda, const double* host_in,
                                   double* host_out, void* stream);
 
+/* ---- form of the affine simplex operators ------------------------------------------------------
+ * With constant dxi/dx and |J| the operators of Eq. 6-7 are (L + lambda M)_e = sum_{c<6} G^e_c K_c +
+ * lambda |J_e| K_6 with seven Nm x Nm matrices of the STANDARD element (the quadrature sums of Eq. 7 with the chain of
+ * Eq. 23 applied to the basis, taken over the points first) and the element's metric G^e = |J| (dxi/dx)(dxi/dx)^T:
+ * a dense GEMM with a fixed right-hand matrix, run on the FP64 tensor cores (DMMA) for tets up to P = 5 where it
+ * needs fewer flops than the sum-factorised chain.  nk_mass_apply, nk_laplacian_apply and every
+ * nk_helmholtz_* call on an AFFINE simplex block take
+ *   form 0 (default)  the reference-matrix kernel where one is instantiated (tets), else the sum-factorised kernel,
+ *   form 1            the sum-factorised kernel (Eq. 17 / 21 / 23 step by step, as on deformed blocks),
+ *   form 2            the reference-matrix kernel; NK_ERR_UNSUPPORTED at apply time where none is instantiated.
+ * Process-wide; the initial value is the environment variable NK_SIMPLEX_FORM (0 if unset).                     */
+nk_status nk_set_affine_simplex_form(int form);
+int nk_get_affine_simplex_form(void);
+/* matrix c = 0..6 of the standard element, [Nm][Nm] row-major, symmetric (host memory, cap in doubles >= Nm^2):
+ * c = 0 (1,1), 1 (1,2)+(2,1), 2 (1,3)+(3,1), 3 (2,2), 4 (2,3)+(3,2), 5 (3,3): sum_q w_q d_a phi_m d_b phi_n in
+ * standard-element coordinates; c = 6: sum_q w_q phi_m phi_n.  Built on first use (host only; needs no GPU).   */
+nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, double* host_out, size_t cap);
+
 /* ---- diagnostics ----------------------------------------------------------------------------- */
 /* Register-only DFMA chains on every SM for `iters` x 1024 FMAs per thread (8 independent chains); *tflops receives the
  * sustained fp64 rate (2 flop per FMA).  This is the measured FP64 roofline denominator.            */

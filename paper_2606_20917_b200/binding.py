@@ -42,6 +42,9 @@ _SIG = {
     "nk_helmholtz_apply_fields": (_i, [_p, _p, _d, _i, C.POINTER(_p), C.POINTER(_p), _p]),
     "nk_helmholtz_apply_blocks": (_i, [_i, _p, _d, _p]),
     "nk_helmholtz_apply_host": (_i, [_p, _p, _d, _p, _p, _p]),
+    "nk_set_affine_simplex_form": (_i, [_i]),
+    "nk_get_affine_simplex_form": (_i, []),
+    "nk_basis_get_reference_matrix": (_i, [_p, _i, C.POINTER(_d), _sz]),
     "nk_probe_fp64_peak": (_i, [_i, C.POINTER(_d), C.POINTER(_d)]),
     "nk_launch_count": (_i64, []),
     "nk_last_error": (C.c_char_p, []),
@@ -125,6 +128,13 @@ class Basis:
 
     def mode_index(self, p, q, r):
         return lib.nk_basis_mode_index(self.h, p, q, r)
+
+    def reference_matrix(self, c):
+        """matrix c = 0..6 of the standard element [Nm][Nm] (nk_basis_get_reference_matrix; host only)."""
+        n = self.num_modes * self.num_modes
+        buf = (_d * n)()
+        _check(lib.nk_basis_get_reference_matrix(self.h, c, buf, n))
+        return torch.frombuffer(buf, dtype=torch.float64).clone().reshape(self.num_modes, self.num_modes)
 
     def close(self):
         if self.h:
@@ -219,6 +229,15 @@ def helmholtz_apply_host(basis, geom, lam, host_in, host_out, stream=None):
     if host_in.is_cuda or host_out.is_cuda:
         raise ValueError("host tensors required")
     _check(lib.nk_helmholtz_apply_host(basis.h, geom.h, float(lam), _ptr(host_in), _ptr(host_out), _stream(stream)))
+
+
+def set_affine_simplex_form(form):
+    """0 = automatic, 1 = sum-factorised, 2 = reference-matrix (nk_set_affine_simplex_form)."""
+    _check(lib.nk_set_affine_simplex_form(int(form)))
+
+
+def get_affine_simplex_form():
+    return lib.nk_get_affine_simplex_form()
 
 
 def probe_fp64_peak(iters=200):

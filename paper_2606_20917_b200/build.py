@@ -56,6 +56,9 @@ def build(force=False, jobs=None, verbose=False, extra_defs=()):
     tasks = []
     api_o = os.path.join(OBJ, "nk_api.o")
     tasks.append((api_o, [nvcc, *COMMON, *ARCH, "-c", os.path.join(CSRC, "nk_api.cu"), "-o", api_o]))
+    dense_o = os.path.join(OBJ, "nk_dense.o")
+    tasks.append((dense_o, [nvcc, *COMMON, *ARCH, *(["-Xptxas", "-v"] if verbose else []), "-c",
+                            os.path.join(CSRC, "nk_dense.cu"), "-o", dense_o]))
     tab_o = os.path.join(OBJ, "nk_host_tables.o")
     tasks.append((tab_o, [nvcc, *COMMON, "-c", os.path.join(CSRC, "nk_host_tables.cpp"), "-o", tab_o]))
     for shape, pmax in MAX_P.items():

@@ -3,12 +3,14 @@
 #include <algorithm>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
 #include <vector>
 
 #include "../../include/nk.h"
+#include "nk_dense_launch.h"
 #include "nk_host_tables.h"
 #include "nk_launch.h"
 
@@ -48,6 +50,21 @@ InstGetter inst_getter(int shape, int P)
     return tab[shape][P - 1];
 }
 
+// form of the affine simplex operators (mass / Laplacian / Helmholtz): 0 = automatic (reference-matrix DMMA kernel
+// where one is instantiated, else the sum-factorised kernel), 1 = sum-factorised always, 2 = reference-matrix
+// (NK_ERR_UNSUPPORTED where none is instantiated).  Initial value from the environment variable NK_SIMPLEX_FORM.
+int g_simplex_form = -1;
+int simplex_form()
+{
+    std::lock_guard<std::mutex> lk(g_mutex);
+    if (g_simplex_form < 0) {
+        const char* ev = std::getenv("NK_SIMPLEX_FORM");
+        const int v = ev ? std::atoi(ev) : 0;
+        g_simplex_form = (v >= 0 && v <= 2) ? v : 0;
+    }
+    return g_simplex_form;
+}
+
 int g_num_sms = 0;
 nk_status ensure_device()
 {
@@ -70,7 +87,59 @@ struct nk_basis {
     std::vector<double> tabs_flat; // DenseTabs<nm,Q> in declaration order
     std::vector<double> sx_flat;   // SimplexTabs in declaration order (simplices only)
     std::vector<double> kron[3];   // hex: the 1-D matrices M, K, C of the coefficient-space forms (NK_TAB_KRON)
+    // reference-matrix form of the affine operators (nk_dense.cuh): built on first use, under `mu`
+    mutable std::mutex mu;
+    mutable std::vector<double> refmat;                              // K7[7][Nm][Nm]
+    mutable double* d_frag[nk::DENSE_KINDS] = {nullptr, nullptr, nullptr}; // fragment-ordered device copies per operator kind
+    mutable int frag_dev = -1;                                       // device ordinal the copies live on
 };
+
+namespace {
+const std::vector<double>& reference_matrices(const nk_basis* b)
+{
+    std::lock_guard<std::mutex> lk(b->mu);
+    if (b->refmat.empty()) nk::build_reference_matrices(b->t, b->refmat);
+    return b->refmat;
+}
+// device copy of the fragment-ordered matrices of one operator kind (lazily, once per basis)
+nk_status dense_fragments(const nk_basis* b, int kind, const double** out)
+{
+    const std::vector<double>& K7 = reference_matrices(b);
+    std::lock_guard<std::mutex> lk(b->mu);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice");
+    if (b->frag_dev >= 0 && b->frag_dev != dev)
+        return fail(NK_ERR_UNSUPPORTED, "this basis already holds device tables on another GPU: create one nk_basis per device");
+    if (!b->d_frag[kind]) {
+        const int c0 = nk::dense_c0(kind), nc = nk::dense_nc(kind);
+        std::vector<double> frag(nk::dense_pack_size(b->t.Nm, nc));
+        nk::dense_pack(K7.data(), b->t.Nm, c0, nc, frag.data());
+        double* d = nullptr;
+        e = cudaMalloc(&d, frag.size() * sizeof(double));
+        if (e != cudaSuccess) { g_err = "reference matrices: cudaMalloc failed"; return NK_ERR_ALLOC; }
+        e = cudaMemcpy(d, frag.data(), frag.size() * sizeof(double), cudaMemcpyHostToDevice);   // synchronous, once per basis
+        if (e != cudaSuccess) { cudaFree(d); return cuda_fail(e, "reference matrices: upload"); }
+        b->d_frag[kind] = d;
+        b->frag_dev = dev;
+    }
+    *out = b->d_frag[kind];
+    return NK_OK;
+}
+// does this (basis, geometry, operator) take the reference-matrix kernel?  *st receives an error if form 2 is forced
+// where no kernel exists.
+bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
+{
+    *st = NK_OK;
+    if (deformed || b->t.shape == nk::HEX) return false;
+    if (op != nk::OP_MASS && op != nk::OP_LAP && op != nk::OP_HELM && op != nk::OP_HELMF) return false;
+    const int form = simplex_form();
+    if (form == 1) return false;
+    const bool have = nk::dense_supported(b->t.Nm) && (b->t.shape == nk::TET || form == 2);
+    if (!have && form == 2) *st = fail(NK_ERR_UNSUPPORTED, "no reference-matrix kernel for this (shape, P)");
+    return have;
+}
+} // namespace
 
 struct nk_geom {
     const nk_basis* b = nullptr;
@@ -172,6 +241,8 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
 extern "C" nk_status nk_basis_destroy(nk_basis* b)
 {
     if (!b) return NK_OK;
+    for (int k = 0; k < nk::DENSE_KINDS; ++k)
+        if (b->d_frag[k]) cudaFree(b->d_frag[k]);
     delete b;
     return NK_OK;
 }
@@ -434,6 +505,35 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     }
     nk_status st = ensure_device();
     if (st != NK_OK) return st;
+    if (g && use_dense(b, g->deformed, op, &st)) {
+        // affine simplex mass / Laplacian / Helmholtz in coefficient space on the FP64 tensor cores (nk_dense.cuh);
+        // group0 / group_count are in tiles of 8 elements here (dense_tile_elems)
+        if (!g->d_metric) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": this geometry was uploaded without NK_GEOM_METRIC");
+        const int kind = op == nk::OP_MASS ? nk::DENSE_MASS : op == nk::OP_LAP ? nk::DENSE_LAP : nk::DENSE_HELM;
+        nk::DenseArgs d;
+        st = dense_fragments(b, kind, &d.bfrag);
+        if (st != NK_OK) return st;
+        d.geom = g->d_metric;
+        d.EG = g->E;
+        d.EGshift = 0;
+        while ((1 << d.EGshift) < g->E) ++d.EGshift;
+        if ((1 << d.EGshift) != g->E) return fail(NK_ERR_UNSUPPORTED, std::string(name) + ": interleave width is not a power of two");
+        d.nfields = fin ? nfields : 1;
+        for (int f = 0; f < nk::DENSE_MAX_FIELDS; ++f) {
+            d.in[f] = (fin && f < nfields) ? fin[f] : in0;
+            d.out[f] = (fout && f < nfields) ? fout[f] : out0;
+        }
+        d.e0 = group0 * 8;
+        d.e1 = group_count < 0 ? nelem : std::min<int64_t>(nelem, (group0 + group_count) * 8);
+        if (d.e0 < 0 || d.e0 > nelem) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": bad tile range");
+        d.scale6 = (kind == nk::DENSE_MASS) ? 1.0 : lambda;
+        int launched = 0;
+        cudaError_t e = nk::dense_launch(b->t.Nm, kind, d, (cudaStream_t)stream, &launched);
+        if (e != cudaSuccess) return cuda_fail(e, name);
+        if (launched) { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
+        return NK_OK;
+    }
+    if (st != NK_OK) return st;
     const int E = (g && g->deformed) ? b->inst->E[1] : b->inst->E_op_affine[op];
     nk::KArgs a;
     a.in[0] = in0; a.in[1] = in1; a.in[2] = in2;
@@ -547,7 +647,11 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
         }
         if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: stream / event creation");
     }
-    const int Eop = g->deformed ? b->inst->E[1] : b->inst->E_op_affine[nk::OP_HELM];   // groups of the kernel, not of the stream
+    nk_status dst = NK_OK;
+    const bool dense = use_dense(b, g->deformed, nk::OP_HELM, &dst);
+    if (dst != NK_OK) return dst;
+    // chunk unit: groups of the kernel (not of the stream), or tiles of 8 elements of the reference-matrix kernel
+    const int Eop = dense ? 8 : g->deformed ? b->inst->E[1] : b->inst->E_op_affine[nk::OP_HELM];
     const int64_t ngroups_op = (g->nelem + Eop - 1) / Eop;
     const int64_t per = (ngroups_op + nk_geom::kChunks - 1) / nk_geom::kChunks;
     const size_t elem_bytes = (size_t)b->t.Nm * sizeof(double);
@@ -576,6 +680,27 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
     if (e == cudaSuccess) e = cudaStreamWaitEvent(s, g->ev_done, 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
     if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: synchronise");
+    return NK_OK;
+}
+
+// =========================== options ===========================
+extern "C" nk_status nk_set_affine_simplex_form(int form)
+{
+    if (form < 0 || form > 2) return fail(NK_ERR_INVALID_ARG, "nk_set_affine_simplex_form: form must be 0 (auto), 1 (sum-factorised) or 2 (reference-matrix)");
+    simplex_form();      // reads the environment default first
+    std::lock_guard<std::mutex> lk(g_mutex);
+    g_simplex_form = form;
+    return NK_OK;
+}
+extern "C" int nk_get_affine_simplex_form(void) { return simplex_form(); }
+
+extern "C" nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, double* host_out, size_t cap)
+{
+    if (!b || c < 0 || c > 6 || !host_out) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_reference_matrix: bad arguments");
+    const size_t n = (size_t)b->t.Nm * b->t.Nm;
+    if (cap < n) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_reference_matrix: capacity too small");
+    const std::vector<double>& K7 = reference_matrices(b);
+    std::memcpy(host_out, K7.data() + (size_t)c * n, n * sizeof(double));
     return NK_OK;
 }
 

@@ -5,7 +5,7 @@
 //             guesses; GRJ: Newton with deflation on P^{alpha,1}_{Q-1}
 //   weights   closed forms (A9), not the interpolatory integral
 //   D         barycentric formula, not the Lagrange product formula
-// so that the table-level parity test (tests/test_tables.py) is a real check.
+// so that the table-level parity test (tests/test_library_cpu.py) is a real check.
 #include "nk_host_tables.h"
 
 #include <cmath>
@@ -242,6 +242,108 @@ bool build_host_tables(int shape, int P, int Q, HostTables& t)
         t.n1 = nm * nm;
     }
     return true;
+}
+
+// ---- reference-element matrices of the coefficient-space form (affine elements) ------------
+// Every basis function is evaluated at every quadrature point as the product of its three 1-D factors
+// (A7) with the top-vertex / top-edge corrections of A8 written out as their definition (factor 1 instead
+// of psi^a_0, or of psi^a_0 psi^b_00); its eta-derivatives are taken with the collocation matrices of
+// Eq. 22, exactly as the kernels differentiate point values, and mapped to xi-derivatives by Eq. 23 (A17).
+void build_reference_matrices(const HostTables& t, std::vector<double>& K7)
+{
+    const int Q = t.Q, nm = t.nm, Nm = t.Nm, Nq = t.Nq;
+    std::vector<double> phi((size_t)Nq * Nm, 0.0);
+    auto pt = [Q](int i, int j, int k) { return (size_t)i + (size_t)Q * (j + (size_t)Q * k); };
+    for (int p = 0; p < nm; ++p) {
+        const int nq2 = t.shape == TET ? nm - p : nm;
+        for (int q = 0; q < nq2; ++q) {
+            const int nr = t.shape == HEX ? nm : t.shape == TET ? nm - p - q : nm - p;
+            for (int r = 0; r < nr; ++r) {
+                const int m = mode_index(t.shape, nm, p, q, r);
+                for (int k = 0; k < Q; ++k)
+                    for (int j = 0; j < Q; ++j)
+                        for (int i = 0; i < Q; ++i) {
+                            double fa = t.psi[0][(size_t)i * nm + p], fb, fc;
+                            if (t.shape == HEX) {
+                                fb = t.psi[1][(size_t)j * nm + q];
+                                fc = t.psi[2][(size_t)k * nm + r];
+                            } else if (t.shape == TET) {
+                                fb = t.psi[1][(size_t)j * t.npair + pair_index(nm, p, q)];
+                                fc = t.psi[2][(size_t)k * t.npair + pair_index(nm, p + q, r)];
+                                if (p == 0 && q == 1) fa = 1.0;                       // A8: top edge
+                                if (p == 0 && q == 0 && r == 1) { fa = 1.0; fb = 1.0; } // A8: top vertex
+                            } else {
+                                fb = t.psi[1][(size_t)j * nm + q];
+                                fc = t.psi[2][(size_t)k * t.npair + pair_index(nm, p, r)];
+                                if (p == 0 && r == 1) fa = 1.0;                       // A8: top edge of the prism
+                            }
+                            phi[pt(i, j, k) * Nm + m] = fa * fb * fc;
+                        }
+            }
+        }
+    }
+    // xi-derivatives, one direction at a time: g[d][n][m]
+    std::vector<double> g[3];
+    for (int d = 0; d < 3; ++d) g[d].assign((size_t)Nq * Nm, 0.0);
+    std::vector<double> e1((size_t)Nm), e2((size_t)Nm), e3((size_t)Nm);
+    for (int k = 0; k < Q; ++k)
+        for (int j = 0; j < Q; ++j)
+            for (int i = 0; i < Q; ++i) {
+                for (int m = 0; m < Nm; ++m) e1[m] = e2[m] = e3[m] = 0.0;
+                for (int r = 0; r < Q; ++r) {
+                    const double a = t.D[0][(size_t)i * Q + r], b = t.D[1][(size_t)j * Q + r], c = t.D[2][(size_t)k * Q + r];
+                    const double *f1 = &phi[pt(r, j, k) * Nm], *f2 = &phi[pt(i, r, k) * Nm], *f3 = &phi[pt(i, j, r) * Nm];
+                    for (int m = 0; m < Nm; ++m) {
+                        e1[m] += a * f1[m];
+                        e2[m] += b * f2[m];
+                        e3[m] += c * f3[m];
+                    }
+                }
+                const double z1 = t.z[0][i], z2 = t.z[1][j], z3 = t.z[2][k];
+                double *x1 = &g[0][pt(i, j, k) * Nm], *x2 = &g[1][pt(i, j, k) * Nm], *x3 = &g[2][pt(i, j, k) * Nm];
+                for (int m = 0; m < Nm; ++m) {
+                    if (t.shape == TET) {
+                        const double c1 = 4.0 / ((1.0 - z2) * (1.0 - z3)), c2 = 2.0 * (1.0 + z1) / ((1.0 - z2) * (1.0 - z3));
+                        const double c3 = 2.0 / (1.0 - z3), c4 = (1.0 + z2) / (1.0 - z3);
+                        x1[m] = c1 * e1[m];
+                        x2[m] = c2 * e1[m] + c3 * e2[m];
+                        x3[m] = c2 * e1[m] + c4 * e2[m] + e3[m];
+                    } else if (t.shape == PRISM) {
+                        x1[m] = 2.0 / (1.0 - z3) * e1[m];
+                        x2[m] = e2[m];
+                        x3[m] = (1.0 + z1) / (1.0 - z3) * e1[m] + e3[m];
+                    } else {
+                        x1[m] = e1[m];
+                        x2[m] = e2[m];
+                        x3[m] = e3[m];
+                    }
+                }
+            }
+    K7.assign((size_t)7 * Nm * Nm, 0.0);
+    const size_t MM = (size_t)Nm * Nm;
+    for (int k = 0; k < Q; ++k)
+        for (int j = 0; j < Q; ++j)
+            for (int i = 0; i < Q; ++i) {
+                const double w = t.w[0][i] * t.w[1][j] * t.w[2][k];
+                const size_t n = pt(i, j, k) * Nm;
+                const double *f = &phi[n], *x1 = &g[0][n], *x2 = &g[1][n], *x3 = &g[2][n];
+                for (int m = 0; m < Nm; ++m) {
+                    const double wf = w * f[m], w1 = w * x1[m], w2 = w * x2[m], w3 = w * x3[m];
+                    double* row = &K7[(size_t)m * Nm];
+                    for (int c = 0; c <= m; ++c) { // lower triangle; mirrored below
+                        row[0 * MM + c] += w1 * x1[c];
+                        row[1 * MM + c] += w1 * x2[c] + w2 * x1[c];
+                        row[2 * MM + c] += w1 * x3[c] + w3 * x1[c];
+                        row[3 * MM + c] += w2 * x2[c];
+                        row[4 * MM + c] += w2 * x3[c] + w3 * x2[c];
+                        row[5 * MM + c] += w3 * x3[c];
+                        row[6 * MM + c] += wf * f[c];
+                    }
+                }
+            }
+    for (int c = 0; c < 7; ++c)
+        for (int m = 0; m < Nm; ++m)
+            for (int n = m + 1; n < Nm; ++n) K7[c * MM + (size_t)m * Nm + n] = K7[c * MM + (size_t)n * Nm + m];
 }
 
 } // namespace nk

@@ -34,4 +34,13 @@ int num_modes(int shape, int nm);
 // returns false if (shape,P,Q) is malformed (P<1, Q<2)
 bool build_host_tables(int shape, int P, int Q, HostTables& t);
 
+// Reference-element matrices of the coefficient-space form of the AFFINE operators (csrc/nk_dense.cuh):
+// K7[c][m][n], c = 0..6, each Nm x Nm row-major and symmetric, with xi = standard-element coordinates,
+//   c = 0: (1,1)  1: (1,2)+(2,1)  2: (1,3)+(3,1)  3: (2,2)  4: (2,3)+(3,2)  5: (3,3):
+//          sum_q w_q d_a phi_m(xi_q) d_b phi_n(xi_q)   (Eq. 7, with the chain of Eq. 23, applied to the basis)
+//   c = 6: sum_q w_q phi_m(xi_q) phi_n(xi_q)            (M = B^T w B, Eq. 7)
+// the same discrete quadrature sums as the sum-factorised chain (w includes the collapse Jacobian, A16), so that
+// (L + lambda M)_e = sum_{c<6} G^e_c K_c + lambda |J_e| K_6 for an element with constant metric G^e = |J| A A^T.
+void build_reference_matrices(const HostTables& t, std::vector<double>& K7);
+
 } // namespace nk

@@ -20,6 +20,20 @@ def nk():
     return nk
 
 
+import contextlib
+
+
+@contextlib.contextmanager
+def simplex_form(nk, form):
+    """forces the form of the affine simplex operators (nk_set_affine_simplex_form) for the duration of a block"""
+    old = nk.get_affine_simplex_form()
+    nk.set_affine_simplex_form(form)
+    try:
+        yield
+    finally:
+        nk.set_affine_simplex_form(old)
+
+
 def run_case(nk, shape, P, n, deformed, ops, lam=1.0, take=None, seed=wl.SEED0, zhi=None):
     el = K.element(shape, P)
     A, J = K.geometry(shape, P, n, deformed, take=take, zhi=zhi)
@@ -53,9 +67,25 @@ def test_all_ops_P4_ragged(nk, shape, deformed):
     run_case(nk, shape, 4, 3, deformed, K.OPS, lam=1.0, take=take, seed=wl.SEED0 + 2)
 
 
+@pytest.mark.parametrize("shape", [o.TET, o.PRISM])
+def test_all_ops_P4_ragged_sum_factorised_form(nk, shape):
+    """the same on affine simplices with the sum-factorised kernels forced (form 1; the default on affine tets
+    is the reference-matrix kernel)."""
+    full = K.mesh(shape, 3)[0].shape[0]
+    with simplex_form(nk, 1):
+        run_case(nk, shape, 4, 3, False, K.OPS, lam=1.0, take=torch.arange(full - 5), seed=wl.SEED0 + 2)
+
+
 @pytest.mark.parametrize("P", range(1, 11))
 def test_config4_hex_psweep_mass_laplacian(nk, P):
     run_case(nk, o.HEX, P, 3 if P < 8 else 2, False, ("mass", "laplacian"), seed=wl.SEED0 + 4)
+
+
+@pytest.mark.parametrize("P", range(1, 11))
+def test_hex_affine_all_orders_helmholtz_bwd_iprod(nk, P):
+    """Helmholtz (lambda != 1) on AFFINE hexes at every order: the coefficient-space kernel (nk_stage_lapkron.inc)
+    with its lambda |J| term on both sides of the NK_LAPKRON_MAXNM switch, plus BwdTrans / IProduct at every order."""
+    run_case(nk, o.HEX, P, 3 if P < 8 else 2, False, ("helmholtz", "bwdtrans", "iprod"), lam=2.75, seed=wl.SEED0 + 14)
 
 
 @pytest.mark.parametrize("P", range(1, 11))
@@ -69,6 +99,57 @@ def test_simplex_all_orders(nk, shape, P):
     for deformed in (False, True):
         run_case(nk, shape, P, 2, deformed, ("bwdtrans", "iprod", "helmholtz", "physderiv", "iprod_deriv"),
                  lam=10.0, seed=wl.SEED0 + 5, zhi=1)
+
+
+@pytest.mark.parametrize("shape", [o.TET, o.PRISM])
+@pytest.mark.parametrize("P", [1, 2, 3])
+def test_simplex_low_order_full_groups_and_tail(nk, shape, P):
+    """low orders have wide interleaves (32 at P1 affine): at least two full groups plus a ragged tail."""
+    full = K.mesh(shape, 4)[0].shape[0]          # 384 tets / 128 prisms
+    take = torch.arange(full - 3)
+    for deformed in (False, True):
+        for form in ((1, 0) if not deformed else (0,)):
+            with simplex_form(nk, form):
+                run_case(nk, shape, P, 4, deformed, ("bwdtrans", "iprod", "mass", "laplacian", "helmholtz"), lam=0.3,
+                         take=take, seed=wl.SEED0 + 15)
+
+
+@pytest.mark.parametrize("P", range(1, 9))
+def test_affine_tet_reference_matrix_form(nk, P):
+    """the reference-matrix (DMMA) kernels of nk_dense.cuh against the oracle: mass, Laplacian, Helmholtz with
+    lambda != 1 on several tiles of 8 elements plus a ragged tail, and against the sum-factorised form."""
+    if not _dense_available(nk, o.TET, P):
+        pytest.skip("no reference-matrix kernel instantiated for tet P%d" % P)
+    el = K.element(o.TET, P)
+    full = K.mesh(o.TET, 3 if P < 7 else 2)[0].shape[0]        # 162 / 48 tets
+    for ne in (full - 3, 8, 1):
+        A, J = K.geometry(o.TET, P, 3 if P < 7 else 2, False, take=torch.arange(ne))
+        basis = nk.Basis(o.TET, P)
+        geom = nk.Geom(basis, A.cuda(), J.cuda(), False)
+        for op in ("mass", "laplacian", "helmholtz"):
+            x = K.make_input(op, wl.SEED0 + 16, ne, el)
+            ref = K.oracle_op(op, el, A, J, 3.25, x)
+            with simplex_form(nk, 2):
+                got = K.gpu_op(nk, op, basis, geom, 3.25, x)
+            with simplex_form(nk, 1):
+                sf = K.gpu_op(nk, op, basis, geom, 3.25, x)
+            assert K.normwise_err(got, ref) <= TOL, (P, ne, op)
+            assert K.normwise_err(sf, ref) <= TOL, (P, ne, op)
+            assert K.normwise_err(got, sf) <= 1e-13, (P, ne, op)
+
+
+def _dense_available(nk, shape, P):
+    basis = nk.Basis(shape, P)
+    A, J = K.geometry(shape, P, 2, False, take=torch.arange(1))
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), False)
+    x = torch.zeros((1, basis.num_modes), dtype=torch.float64, device="cuda")
+    with simplex_form(nk, 2):
+        try:
+            nk.mass_apply(basis, geom, x, torch.empty_like(x))
+        except nk.NkError as e:
+            assert e.code == 2          # NK_ERR_UNSUPPORTED is the only acceptable refusal
+            return False
+    return True
 
 
 def test_config5_blocks_small(nk):
@@ -150,6 +231,23 @@ def test_operator_identities_on_gpu(nk):
         assert K.normwise_err(l1, l2) <= 1e-13
         h = K.gpu_op(nk, "helmholtz", basis, geom, lam, x)
         assert K.normwise_err(h, l2 + lam * m2) <= 1e-13
+
+
+def test_helmholtz_host_entry_affine_tet(nk):
+    """host entry on the reference-matrix kernel: the chunks of the pipeline are tiles of 8 elements."""
+    P = 4
+    el = K.element(o.TET, P)
+    full = K.mesh(o.TET, 3)[0].shape[0]
+    A, J = K.geometry(o.TET, P, 3, False, take=torch.arange(full - 3))
+    basis = nk.Basis(o.TET, P)
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), False)
+    x = wl.coefficients(22, J.shape[0], el.Nm).pin_memory()
+    ref = o.helmholtz(el, A.numpy(), J.numpy(), 1.5, x.numpy())
+    for form in (0, 1):
+        y = torch.full_like(x, float("nan")).pin_memory()
+        with simplex_form(nk, form):
+            nk.helmholtz_apply_host(basis, geom, 1.5, x, y)
+        assert K.normwise_err(y.numpy(), ref) <= TOL
 
 
 @pytest.mark.parametrize("deformed", [True, False])

@@ -123,3 +123,40 @@ def test_kronecker_matrices_of_the_affine_hex_forms():
         np.testing.assert_allclose(C + C.T, bnd, atol=1e-13)
     with pytest.raises(nk.NkError):
         nk.Basis(o.TET, 3).table(nk.TAB_KRON, 0)
+
+
+@pytest.mark.parametrize("shape,P", [(o.TET, 1), (o.TET, 2), (o.TET, 3), (o.TET, 4), (o.TET, 5), (o.TET, 7), (o.PRISM, 2), (o.PRISM, 4),
+                                     (o.HEX, 2)])
+def test_reference_matrices_match_oracle(shape, P):
+    """nk_basis_get_reference_matrix (host side of the reference-matrix kernels, csrc/nk_dense.cuh): the seven
+    matrices of the standard element, combined with the metric of a random affine element, give the oracle's
+    elemental Helmholtz matrix (built column by column by the oracle's dense quadrature sums)."""
+    rng = np.random.default_rng(1000 * shape + P)
+    el = o.Element(shape, P, P + 2)
+    b = nk.Basis(shape, P)
+    K = [b.reference_matrix(c).numpy() for c in range(7)]
+    for k in K:
+        assert np.array_equal(k, k.T)
+    A = rng.standard_normal((1, 1, 3, 3)) + 2.0 * np.eye(3)
+    J = np.array([[1.7]])
+    lam = 1.3
+    ref = np.stack([o.helmholtz(el, A, J, lam, np.eye(el.Nm)[i:i + 1])[0] for i in range(el.Nm)], axis=1)
+    G = J[0, 0] * A[0, 0] @ A[0, 0].T
+    H = (G[0, 0] * K[0] + G[0, 1] * K[1] + G[0, 2] * K[2] + G[1, 1] * K[3] + G[1, 2] * K[4] + G[2, 2] * K[5]
+         + lam * J[0, 0] * K[6])
+    assert np.abs(H - ref).max() <= 1e-13 * np.abs(ref).max()
+    # the mass matrix alone, and the Laplacian annihilates constants (vertex modes sum to 1: A8)
+    M = np.stack([o.mass(el, J, np.eye(el.Nm)[i:i + 1])[0] for i in range(el.Nm)], axis=1)
+    assert np.abs(J[0, 0] * K[6] - M).max() <= 1e-13 * np.abs(M).max()
+
+
+def test_simplex_form_option():
+    old = nk.get_affine_simplex_form()
+    try:
+        for f in (0, 1, 2):
+            nk.set_affine_simplex_form(f)
+            assert nk.get_affine_simplex_form() == f
+        with pytest.raises(nk.NkError):
+            nk.set_affine_simplex_form(3)
+    finally:
+        nk.set_affine_simplex_form(old)
