@@ -207,6 +207,208 @@ __global__ void __launch_bounds__(WARPS * 32, MINB) nk_dense_kernel(const __grid
     }
 }
 
+// ---- streamed variant for the orders whose matrices do not fit shared memory (tets P >= 6: Nm = 84, 120, 165) ----
+// The same GEMM; the fragment-ordered matrices stay in L2 (1.6 MB at P8) and are streamed through a ring of STAGES
+// shared-memory chunks of KSC k-steps each by a producer warp (TMA bulk copies, mbarrier full / empty pairs), while
+// WARPS consumer warps, one tile of 8 elements each, walk over the chunks in step: every chunk read from L2 serves
+// WARPS x 8 elements.  Coefficients and metric weights of a tile sit in a per-warp shared-memory slab (the A
+// fragments are one LDS per k-step), so that only the accumulators live in registers.
+template <int NMODES, int C0, int NC, int KSC>
+struct DenseStream {
+    using S = DenseShape<NMODES, C0, NC>;
+    static_assert(S::NK % KSC == 0, "KSC must divide the number of k-steps");
+    static constexpr int KB = S::NK / KSC;                               // chunks per matrix
+    static constexpr int MAIN_CHUNKS = S::NTS > 0 ? NC * KB : 0, REM_CHUNKS = S::NRT > 0 ? KB : 0;
+    static constexpr int CHUNKS = MAIN_CHUNKS + REM_CHUNKS;             // per tile
+    static constexpr int MAIN_CHUNK_DOUBLES = KSC * S::NTS * 32, REM_CHUNK_DOUBLES = KSC * S::NRT * 32;
+    static constexpr int STAGE_DOUBLES = MAIN_CHUNK_DOUBLES > REM_CHUNK_DOUBLES ? MAIN_CHUNK_DOUBLES : REM_CHUNK_DOUBLES;
+    static constexpr int USTRIDE = (4 * S::NK) % 8 == 4 ? 4 * S::NK : 4 * S::NK + 4;   // = 4 mod 8: conflict-free A reads
+    static constexpr int SLAB_DOUBLES = 8 * USTRIDE + 64;               // u[8][USTRIDE] + g[8][8]
+    static constexpr size_t smem_bytes(int warps, int stages)
+    {
+        return ((size_t)stages * STAGE_DOUBLES + (size_t)warps * SLAB_DOUBLES) * sizeof(double) + 2 * stages * sizeof(unsigned long long);
+    }
+};
+
+__device__ __forceinline__ void mbar_arrive(unsigned long long* bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"((unsigned)__cvta_generic_to_shared(bar)) : "memory");
+}
+
+// A consumer warp hands a ring slot back to the producer.  The fence is REQUIRED: mbarrier.arrive may be performed
+// while this warp's last LDS of the slot are still in flight (ptxas puts the arrive right behind the last load, in
+// front of the DMMA that consume it), and the producer's next TMA copy into the slot then overtakes them -- measured
+// on B200 as stale chunk tails in 1 tile out of ~10 (profiles/r2_dmma.md).  MEMBAR.CTA waits for the warp's
+// outstanding shared-memory reads; the DMMA that use them may still follow it.
+__device__ __forceinline__ void release_slot(unsigned long long* bar, int lane)
+{
+    __threadfence_block();
+    __syncwarp();
+    if (lane == 0) mbar_arrive(bar);
+}
+
+template <int NMODES, int C0, int NC, int WARPS, int KSC, int STAGES, int MINB>
+__global__ void __launch_bounds__((WARPS + 1) * 32, MINB) nk_dense_stream_kernel(const __grid_constant__ DenseArgs a)
+{
+    using S = DenseShape<NMODES, C0, NC>;
+    using T = DenseStream<NMODES, C0, NC, KSC>;
+    constexpr int NK = S::NK, NTS = S::NTS, NRT = S::NRT, NTF = S::NTF, KB = T::KB;
+    extern __shared__ __align__(128) double smem[];
+    double* ring = smem;                                                   // [STAGES][STAGE_DOUBLES]
+    double* slabs = smem + (size_t)STAGES * T::STAGE_DOUBLES;              // [WARPS][SLAB_DOUBLES]
+    unsigned long long* full = reinterpret_cast<unsigned long long*>(slabs + (size_t)WARPS * T::SLAB_DOUBLES);
+    unsigned long long* empty = full + STAGES;
+    if (threadIdx.x == 0) {
+#pragma unroll
+        for (int s = 0; s < STAGES; ++s) {
+            mbar_init(&full[s], 1);
+            mbar_init(&empty[s], WARPS);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const unsigned tpf = (unsigned)((a.e1 - a.e0 + 8 * WARPS - 1) / (8 * WARPS));   // block-tiles (WARPS x 8 elements) per field
+    const unsigned ntiles = tpf * (unsigned)a.nfields;
+    const unsigned my_tiles = blockIdx.x < ntiles ? (ntiles - blockIdx.x + gridDim.x - 1) / gridDim.x : 0u;
+
+    if (warp == WARPS) {
+        // ---- producer: one lane streams the chunk sequence of every tile of this block through the ring ----
+        if (lane == 0) {
+            unsigned n = 0;                                                // chunks issued so far
+            for (unsigned t = 0; t < my_tiles; ++t) {
+                for (int ch = 0; ch < T::CHUNKS; ++ch, ++n) {
+                    const unsigned st = n % STAGES, use = n / STAGES;
+                    if (use > 0) mbar_wait(&empty[st], (use - 1) & 1);
+                    const bool main = ch < T::MAIN_CHUNKS;
+                    const unsigned bytes = (main ? T::MAIN_CHUNK_DOUBLES : T::REM_CHUNK_DOUBLES) * sizeof(double);
+                    const double* src = main ? a.bfrag + (size_t)ch * T::MAIN_CHUNK_DOUBLES
+                                             : a.bfrag + S::MAIN_DOUBLES + (size_t)(ch - T::MAIN_CHUNKS) * T::REM_CHUNK_DOUBLES;
+                    mbar_expect_tx(&full[st], bytes);
+                    bulk_g2s(ring + (size_t)st * T::STAGE_DOUBLES, src, bytes, &full[st]);
+                }
+            }
+        }
+        return;
+    }
+    // ---- consumers ----
+    const int er = lane >> 2, kc = lane & 3;
+    double* __restrict__ us = slabs + (size_t)warp * T::SLAB_DOUBLES;     // u[8][USTRIDE]
+    double* __restrict__ gs = us + 8 * T::USTRIDE;                         // g[8][8]
+    unsigned n = 0;
+    for (unsigned t = 0; t < my_tiles; ++t) {
+        const unsigned tile = blockIdx.x + t * gridDim.x;
+        const unsigned f = a.nfields > 1 ? tile / tpf : 0u;
+        const long long el0 = a.e0 + ((long long)(tile - f * tpf) * WARPS + warp) * 8;
+        // slab: coefficients of 8 elements (coalesced row by row, zero-padded; cp.async, every copy in flight at once:
+        // a load -> store loop serialises 48 DRAM round trips, 13 % of the kernel in ncu) and their metric weights
+        __syncwarp();
+        {
+            constexpr int PER_ROW = (T::USTRIDE + 31) / 32;
+#pragma unroll
+            for (int i = 0; i < 8 * PER_ROW; ++i) {
+                const int r = i / PER_ROW, m = (i % PER_ROW) * 32 + lane;
+                const long long el = el0 + r;
+                const bool ok = el < a.e1 && m < NMODES;
+                if (m < T::USTRIDE) {
+                    const unsigned d = (unsigned)__cvta_generic_to_shared(&us[r * T::USTRIDE + m]);
+                    const double* src = ok ? a.in[f] + el * NMODES + m : a.in[f];
+                    asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(src), "r"(ok ? 8 : 0) : "memory");
+                }
+            }
+        }
+        if (lane < 8) {
+            const long long el = el0 + lane;
+            const long long ee = el < a.e1 ? el : a.e0;
+            const double* __restrict__ gp = a.geom + (ee >> a.EGshift) * (7 * a.EG) + (ee & (a.EG - 1));
+#pragma unroll
+            for (int c = 0; c < 8; ++c) {
+                double v = c < NC ? __ldg(gp + (C0 + c) * a.EG) : 0.0;
+                if (C0 + c == 6) v *= a.scale6;
+                gs[lane * 8 + c] = v;
+            }
+        }
+        {
+            // the next tile's rows (contiguous) -> L2 while this tile is computed
+            const unsigned tn = tile + gridDim.x;
+            if (lane == 0 && t + 1 < my_tiles) {
+                const unsigned fn = a.nfields > 1 ? tn / tpf : 0u;
+                const long long en = a.e0 + ((long long)(tn - fn * tpf) * WARPS + warp) * 8;
+                const long long cnt = a.e1 - en < 8 ? a.e1 - en : 8;
+                const double* p = a.in[fn] + en * NMODES;
+                if (cnt > 0 && (reinterpret_cast<size_t>(p) & 15) == 0) {
+                    const unsigned bytes = (unsigned)(cnt * NMODES * sizeof(double)) & ~15u;
+                    if (bytes) asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+                }
+            }
+        }
+        asm volatile("cp.async.wait_all;" ::: "memory");
+        __syncwarp();
+        double acc[NTS > 0 ? NTS : 1][2], accr[NRT > 0 ? NRT : 1][2];
+#pragma unroll
+        for (int nt = 0; nt < NTS; ++nt) acc[nt][0] = acc[nt][1] = 0.0;
+#pragma unroll
+        for (int rt = 0; rt < NRT; ++rt) accr[rt][0] = accr[rt][1] = 0.0;
+        const double* __restrict__ ul = us + er * T::USTRIDE + kc;
+        if constexpr (NTS > 0) {
+#pragma unroll 1
+            for (int c = 0; c < NC; ++c) {
+                const double gc = gs[er * 8 + c];
+#pragma unroll 1
+                for (int kb = 0; kb < KB; ++kb, ++n) {
+                    const unsigned st = n % STAGES;
+                    mbar_wait(&full[st], (n / STAGES) & 1);
+                    const double* __restrict__ bl = ring + (size_t)st * T::STAGE_DOUBLES + lane;
+#pragma unroll
+                    for (int k = 0; k < KSC; ++k) {
+                        const double as = gc * ul[4 * (kb * KSC + k)];
+#pragma unroll
+                        for (int nt = 0; nt < NTS; ++nt) dmma884(acc[nt][0], acc[nt][1], as, bl[(k * NTS + nt) * 32]);
+                    }
+                    release_slot(&empty[st], lane);
+                }
+            }
+        }
+        if constexpr (NRT > 0) {
+#pragma unroll 1
+            for (int kb = 0; kb < KB; ++kb, ++n) {
+                const unsigned st = n % STAGES;
+                mbar_wait(&full[st], (n / STAGES) & 1);
+                const double* __restrict__ bl = ring + (size_t)st * T::STAGE_DOUBLES + lane;
+#pragma unroll
+                for (int k = 0; k < KSC; ++k) {
+                    const double au = ul[4 * (kb * KSC + k)];
+#pragma unroll
+                    for (int rt = 0; rt < NRT; ++rt) dmma884(accr[rt][0], accr[rt][1], au, bl[(k * NRT + rt) * 32]);
+                }
+                release_slot(&empty[st], lane);
+            }
+        }
+        // ---- store ----
+        const long long el = el0 + er;
+        double* __restrict__ dst = a.out[f] + el * NMODES;
+        const bool ok = el < a.e1;
+        if constexpr (NRT > 0) {
+            const double g0 = gs[er * 8 + 2 * kc], g1 = gs[er * 8 + 2 * kc + 1];
+#pragma unroll
+            for (int rt = 0; rt < NRT; ++rt) {
+                double p = fma(g0, accr[rt][0], g1 * accr[rt][1]);
+                p += __shfl_xor_sync(0xffffffffu, p, 1);
+                p += __shfl_xor_sync(0xffffffffu, p, 2);
+                if (ok && kc == (rt & 3)) dst[8 * NTF + rt] = p;
+            }
+        }
+        if (ok) {
+#pragma unroll
+            for (int nt = 0; nt < NTS; ++nt) {
+                const int m = 8 * nt + 2 * kc;
+                if (8 * nt + 7 < NMODES || m < NMODES) dst[m] = acc[nt][0];
+                if (8 * nt + 7 < NMODES || m + 1 < NMODES) dst[m + 1] = acc[nt][1];
+            }
+        }
+    }
+}
+
 // host: pack the symmetric matrices Kc[c][m][n] (c = 0..6, row-major Nm x Nm each) into fragment order for
 // DenseShape<NMODES, C0, NC>.  out must hold TOTAL_DOUBLES.
 inline void dense_pack(const double* K7, int nmodes, int c0, int nc, double* out)

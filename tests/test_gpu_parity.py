@@ -121,9 +121,9 @@ def test_affine_tet_reference_matrix_form(nk, P):
     if not _dense_available(nk, o.TET, P):
         pytest.skip("no reference-matrix kernel instantiated for tet P%d" % P)
     el = K.element(o.TET, P)
-    full = K.mesh(o.TET, 3 if P < 7 else 2)[0].shape[0]        # 162 / 48 tets
+    full = K.mesh(o.TET, 3)[0].shape[0]        # 162 tets: several tiles of 8 (and of 32 / 64 at P >= 6) plus a tail
     for ne in (full - 3, 8, 1):
-        A, J = K.geometry(o.TET, P, 3 if P < 7 else 2, False, take=torch.arange(ne))
+        A, J = K.geometry(o.TET, P, 3, False, take=torch.arange(ne))
         basis = nk.Basis(o.TET, P)
         geom = nk.Geom(basis, A.cuda(), J.cuda(), False)
         for op in ("mass", "laplacian", "helmholtz"):
