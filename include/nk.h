@@ -145,10 +145,13 @@ nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double 
 
 /* End-to-end variant with HOST field buffers: copies host_in to an internal device buffer, applies the
  * Helmholtz operator and copies the result back into host_out; synchronises `stream` before returning.
- * The work is cut into up to 8 chunks of element groups and pipelined over two internal copy streams, so that
- * the host-to-device copy of one chunk, the kernel of the previous one and the device-to-host copy of the one
- * before overlap (PCIe is full duplex).  Pinned host memory is needed for the overlap; pageable memory works
- * but serialises.                                                                                   */
+ * The work is cut into up to 16 chunks of element groups (at least 2 MB each) and pipelined over two internal copy
+ * streams, so that the host-to-device copy of one chunk, the kernel of the previous one and the device-to-host copy
+ * of the one before overlap (PCIe is full duplex).  Pinned host memory is needed for the overlap; pageable memory
+ * works but serialises.  The staging buffers and the pipeline's streams and events belong to the nk_geom handle
+ * (allocated on first use, freed by nk_geom_destroy): calls on ONE geometry are serialised by a lock inside the
+ * handle, so the call is thread-safe but not concurrent per geometry; use one nk_geom per concurrent caller.
+ * On any error everything that was enqueued is drained before the call returns.                              */
 nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g, double lambda, const double* host_in,
                                   double* host_out, void* stream);
 

@@ -177,34 +177,73 @@ class Geom:
             pass
 
 
+def _field(t, n, what, allow_none=False):
+    """device pointer of a field tensor after checking its size (the C-ABI takes no sizes for field buffers: a
+    short tensor would be a silent out-of-bounds device access) and its device.  Marshalling only."""
+    if t is None:
+        if allow_none:
+            return None
+        raise ValueError("%s: tensor required" % what)
+    if t.numel() != n:
+        raise ValueError("%s holds %d values, the block needs %d" % (what, t.numel(), n))
+    if t.is_cuda and t.device.index != torch.cuda.current_device():
+        raise ValueError("%s lives on cuda:%d, the current device is cuda:%d" % (what, t.device.index, torch.cuda.current_device()))
+    return _dev_ptr(t)
+
+
+def _no_alias(ins, outs):
+    """nk.h: in/out must not alias (checked for every pair here; the library checks the first pair only)."""
+    a = [t.data_ptr() for t in ins if t is not None]
+    b = [t.data_ptr() for t in outs if t is not None]
+    if set(a) & set(b) or len(set(b)) != len(b):
+        raise ValueError("input and output tensors must be distinct buffers")
+
+
 def bwdtrans(basis, coeffs, phys, stream=None):
-    _check(lib.nk_bwdtrans(basis.h, coeffs.shape[0], _dev_ptr(coeffs), _dev_ptr(phys), _stream(stream)))
+    ne = coeffs.shape[0]
+    _no_alias([coeffs], [phys])
+    _check(lib.nk_bwdtrans(basis.h, ne, _field(coeffs, ne * basis.num_modes, "coeffs"),
+                           _field(phys, ne * basis.num_points, "phys"), _stream(stream)))
 
 
 def iprod(basis, geom, phys, coeffs, stream=None):
-    _check(lib.nk_iprod(basis.h, geom.h, _dev_ptr(phys), _dev_ptr(coeffs), _stream(stream)))
+    _no_alias([phys], [coeffs])
+    _check(lib.nk_iprod(basis.h, geom.h, _field(phys, geom.nelem * basis.num_points, "phys"),
+                        _field(coeffs, geom.nelem * basis.num_modes, "coeffs"), _stream(stream)))
 
 
 def physderiv(basis, geom, phys, d0, d1, d2, stream=None):
-    _check(lib.nk_physderiv(basis.h, geom.h, _dev_ptr(phys), _dev_ptr(d0, True), _dev_ptr(d1, True),
-                            _dev_ptr(d2, True), _stream(stream)))
+    nq = geom.nelem * basis.num_points
+    _no_alias([phys], [d0, d1, d2])
+    _check(lib.nk_physderiv(basis.h, geom.h, _field(phys, nq, "phys"), _field(d0, nq, "d0", True), _field(d1, nq, "d1", True),
+                            _field(d2, nq, "d2", True), _stream(stream)))
 
 
 def iprod_deriv(basis, geom, g0, g1, g2, coeffs, stream=None):
-    _check(lib.nk_iprod_deriv(basis.h, geom.h, _dev_ptr(g0, True), _dev_ptr(g1, True), _dev_ptr(g2, True),
-                              _dev_ptr(coeffs), _stream(stream)))
+    nq = geom.nelem * basis.num_points
+    _no_alias([g0, g1, g2], [coeffs])
+    _check(lib.nk_iprod_deriv(basis.h, geom.h, _field(g0, nq, "g0", True), _field(g1, nq, "g1", True), _field(g2, nq, "g2", True),
+                              _field(coeffs, geom.nelem * basis.num_modes, "coeffs"), _stream(stream)))
+
+
+def _coeff_pair(basis, geom, inp, out):
+    n = geom.nelem * geom.basis.num_modes     # sized by the geometry's own basis; a mismatching `basis` is the library's to refuse
+    return _field(inp, n, "in"), _field(out, n, "out")
 
 
 def mass_apply(basis, geom, inp, out, stream=None):
-    _check(lib.nk_mass_apply(basis.h, geom.h, _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+    pi, po = _coeff_pair(basis, geom, inp, out)
+    _check(lib.nk_mass_apply(basis.h, geom.h, pi, po, _stream(stream)))
 
 
 def laplacian_apply(basis, geom, inp, out, stream=None):
-    _check(lib.nk_laplacian_apply(basis.h, geom.h, _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+    pi, po = _coeff_pair(basis, geom, inp, out)
+    _check(lib.nk_laplacian_apply(basis.h, geom.h, pi, po, _stream(stream)))
 
 
 def helmholtz_apply(basis, geom, lam, inp, out, stream=None):
-    _check(lib.nk_helmholtz_apply(basis.h, geom.h, float(lam), _dev_ptr(inp), _dev_ptr(out), _stream(stream)))
+    pi, po = _coeff_pair(basis, geom, inp, out)
+    _check(lib.nk_helmholtz_apply(basis.h, geom.h, float(lam), pi, po, _stream(stream)))
 
 
 def helmholtz_apply_fields(basis, geom, lam, inps, outs, stream=None):
@@ -212,8 +251,9 @@ def helmholtz_apply_fields(basis, geom, lam, inps, outs, stream=None):
     n = len(inps)
     if n != len(outs):
         raise ValueError("as many outputs as inputs")
-    pin = (_p * n)(*[_dev_ptr(t) for t in inps])
-    pout = (_p * n)(*[_dev_ptr(t) for t in outs])
+    nn = geom.nelem * basis.num_modes
+    pin = (_p * n)(*[_field(t, nn, "in[%d]" % k) for k, t in enumerate(inps)])
+    pout = (_p * n)(*[_field(t, nn, "out[%d]" % k) for k, t in enumerate(outs)])
     _check(lib.nk_helmholtz_apply_fields(basis.h, geom.h, float(lam), n, pin, pout, _stream(stream)))
 
 
@@ -221,13 +261,17 @@ def helmholtz_apply_blocks(blocks, lam, stream=None):
     """blocks: sequence of (basis, geom, inp, out)."""
     arr = (NkBlock * len(blocks))()
     for k, (b, g, x, y) in enumerate(blocks):
-        arr[k] = NkBlock(b.h, g.h, _dev_ptr(x), _dev_ptr(y))
+        pi, po = _coeff_pair(b, g, x, y)
+        arr[k] = NkBlock(b.h, g.h, pi, po)
     _check(lib.nk_helmholtz_apply_blocks(len(blocks), arr, float(lam), _stream(stream)))
 
 
 def helmholtz_apply_host(basis, geom, lam, host_in, host_out, stream=None):
     if host_in.is_cuda or host_out.is_cuda:
         raise ValueError("host tensors required")
+    n = geom.nelem * basis.num_modes
+    if host_in.numel() != n or host_out.numel() != n:
+        raise ValueError("host buffers must hold nelem x Nm = %d values" % n)
     _check(lib.nk_helmholtz_apply_host(basis.h, geom.h, float(lam), _ptr(host_in), _ptr(host_out), _stream(stream)))
 
 

@@ -65,17 +65,24 @@ int simplex_form()
     return g_simplex_form;
 }
 
-int g_num_sms = 0;
+// SM count of the CURRENT device (cached per device ordinal)
+thread_local int g_num_sms = 0;
 nk_status ensure_device()
 {
-    if (g_num_sms > 0) return NK_OK;
+    enum { kMaxDevices = 64 };
+    static int sms[kMaxDevices] = {};
     int dev = 0;
     cudaError_t e = cudaGetDevice(&dev);
     if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice (no CUDA device: libnk has no CPU fallback)");
-    int n = 0;
-    e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
-    if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
-    g_num_sms = n;
+    if (dev < 0 || dev >= kMaxDevices) return fail(NK_ERR_UNSUPPORTED, "device ordinal beyond 63");
+    std::lock_guard<std::mutex> lk(g_mutex);
+    if (sms[dev] == 0) {
+        int n = 0;
+        e = cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev);
+        if (e != cudaSuccess) return cuda_fail(e, "cudaDeviceGetAttribute");
+        sms[dev] = n;
+    }
+    g_num_sms = sms[dev];
     return NK_OK;
 }
 
@@ -150,7 +157,8 @@ struct nk_geom {
     // nk_helmholtz_apply_host: device staging buffers and the copy-in / copy-out pipeline
     double* d_stage_in = nullptr;
     double* d_stage_out = nullptr;
-    enum { kChunks = 8 };
+    enum { kChunks = 16 };
+    std::mutex host_mu;          // nk_helmholtz_apply_host is serialised per geometry (one set of staging buffers)
     cudaStream_t s_in = nullptr, s_out = nullptr;
     cudaEvent_t ev_start = nullptr, ev_done = nullptr, ev_in[kChunks] = {}, ev_k[kChunks] = {};
 };
@@ -623,19 +631,38 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
                                              double* host_out, void* stream)
 {
     if (!b || !gc || !host_in || !host_out) return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_host: NULL argument");
-    nk_geom* g = const_cast<nk_geom*>(gc);
+    nk_geom* g = const_cast<nk_geom*>(gc);   // the staging buffers and pipeline objects live in the geometry handle
+    // validate BEFORE anything is allocated: the buffers are sized from the geometry's own basis
+    if (g->b != b && (g->b->t.shape != b->t.shape || g->b->t.P != b->t.P || g->b->t.Q != b->t.Q))
+        return fail(NK_ERR_SHAPE_MISMATCH, "nk_helmholtz_apply_host: geom was uploaded for another basis");
     if (g->nelem == 0) return NK_OK;
-    const size_t bytes = (size_t)g->nelem * b->t.Nm * sizeof(double);
+    if (!g->d_metric) return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_host: this geometry was uploaded without NK_GEOM_METRIC");
+    nk_status dst = ensure_device();
+    if (dst != NK_OK) return dst;
+    const bool dense = use_dense(b, g->deformed, nk::OP_HELM, &dst);
+    if (dst != NK_OK) return dst;
+    std::lock_guard<std::mutex> host_lock(g->host_mu);   // one caller at a time per geometry (documented in nk.h)
+    const int Nm = g->b->t.Nm;
+    const size_t bytes = (size_t)g->nelem * Nm * sizeof(double);
     cudaError_t e = cudaSuccess;
-    if (!g->d_stage_in) {
-        e = cudaMalloc(&g->d_stage_in, bytes);
-        if (e == cudaSuccess) e = cudaMalloc(&g->d_stage_out, bytes);
-        if (e != cudaSuccess) { g_err = "nk_helmholtz_apply_host: cudaMalloc failed"; return NK_ERR_ALLOC; }
+    if (!g->d_stage_in || !g->d_stage_out) {
+        // both buffers or neither
+        double *bi = nullptr, *bo = nullptr;
+        e = cudaMalloc(&bi, bytes);
+        if (e == cudaSuccess) e = cudaMalloc(&bo, bytes);
+        if (e != cudaSuccess) {
+            if (bi) cudaFree(bi);
+            if (bo) cudaFree(bo);
+            cudaGetLastError();
+            g_err = "nk_helmholtz_apply_host: cudaMalloc of the staging buffers failed";
+            return NK_ERR_ALLOC;
+        }
+        g->d_stage_in = bi;
+        g->d_stage_out = bo;
     }
     cudaStream_t s = (cudaStream_t)stream;
-    // Pipeline over chunks of groups: H2D on s_in, the fused kernel on the caller's stream, D2H on s_out, chained
-    // by events, so that the copy-in of chunk c+1 and the copy-out of chunk c-1 (PCIe is full duplex) overlap
-    // the kernel of chunk c.  One cudaMemcpyAsync per chunk and direction.
+    // Pipeline over chunks: H2D on s_in, the fused kernel on the caller's stream, D2H on s_out, chained by events, so
+    // that the copy-in of chunk c+1 and the copy-out of chunk c-1 (PCIe is full duplex) overlap the kernel of chunk c.
     if (!g->s_in) {
         e = cudaStreamCreateWithFlags(&g->s_in, cudaStreamNonBlocking);
         if (e == cudaSuccess) e = cudaStreamCreateWithFlags(&g->s_out, cudaStreamNonBlocking);
@@ -645,41 +672,66 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
             e = cudaEventCreateWithFlags(&g->ev_in[c], cudaEventDisableTiming);
             if (e == cudaSuccess) e = cudaEventCreateWithFlags(&g->ev_k[c], cudaEventDisableTiming);
         }
-        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: stream / event creation");
+        if (e != cudaSuccess) {
+            // leave the handle in the "nothing created" state: the next call starts over
+            if (g->s_in) { cudaStreamDestroy(g->s_in); g->s_in = nullptr; }
+            if (g->s_out) { cudaStreamDestroy(g->s_out); g->s_out = nullptr; }
+            if (g->ev_start) { cudaEventDestroy(g->ev_start); g->ev_start = nullptr; }
+            if (g->ev_done) { cudaEventDestroy(g->ev_done); g->ev_done = nullptr; }
+            for (int c = 0; c < nk_geom::kChunks; ++c) {
+                if (g->ev_in[c]) { cudaEventDestroy(g->ev_in[c]); g->ev_in[c] = nullptr; }
+                if (g->ev_k[c]) { cudaEventDestroy(g->ev_k[c]); g->ev_k[c] = nullptr; }
+            }
+            return cuda_fail(e, "nk_helmholtz_apply_host: stream / event creation");
+        }
     }
-    nk_status dst = NK_OK;
-    const bool dense = use_dense(b, g->deformed, nk::OP_HELM, &dst);
-    if (dst != NK_OK) return dst;
     // chunk unit: groups of the kernel (not of the stream), or tiles of 8 elements of the reference-matrix kernel
     const int Eop = dense ? 8 : g->deformed ? b->inst->E[1] : b->inst->E_op_affine[nk::OP_HELM];
     const int64_t ngroups_op = (g->nelem + Eop - 1) / Eop;
-    const int64_t per = (ngroups_op + nk_geom::kChunks - 1) / nk_geom::kChunks;
-    const size_t elem_bytes = (size_t)b->t.Nm * sizeof(double);
+    // at least ~2 MB per chunk: below that the per-copy latency costs more than the overlap gains
+    int nchunks = (int)std::min<int64_t>(nk_geom::kChunks, std::max<int64_t>(1, (int64_t)(bytes >> 21)));
+    const int64_t per = (ngroups_op + nchunks - 1) / nchunks;
+    const size_t elem_bytes = (size_t)Nm * sizeof(double);
+    nk_status st = NK_OK;
+    const char* what = nullptr;
     e = cudaEventRecord(g->ev_start, s);                  // order after the caller's earlier work on `stream`
     if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_in, g->ev_start, 0);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_out, g->ev_start, 0);
-    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: pipeline start");
-    for (int c = 0; c < nk_geom::kChunks; ++c) {
+    if (e != cudaSuccess) what = "nk_helmholtz_apply_host: pipeline start";
+    for (int c = 0; c < nchunks && e == cudaSuccess && st == NK_OK; ++c) {
         const int64_t g0 = c * per, g1 = std::min<int64_t>(ngroups_op, g0 + per);
         if (g0 >= g1) break;
         const int64_t e0 = g0 * Eop, e1 = std::min<int64_t>(g->nelem, g1 * Eop);
-        const size_t off = (size_t)e0 * b->t.Nm, nb = (size_t)(e1 - e0) * elem_bytes;
+        const size_t off = (size_t)e0 * Nm, nb = (size_t)(e1 - e0) * elem_bytes;
         e = cudaMemcpyAsync(g->d_stage_in + off, host_in + off, nb, cudaMemcpyHostToDevice, g->s_in);
         if (e == cudaSuccess) e = cudaEventRecord(g->ev_in[c], g->s_in);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(s, g->ev_in[c], 0);
-        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: H2D");
-        nk_status st = run_op(nk::OP_HELM, "nk_helmholtz_apply_host", b, g, 0, g->d_stage_in, nullptr, nullptr, g->d_stage_out,
-                              nullptr, nullptr, lambda, stream, 1, nullptr, nullptr, g0, g1 - g0);
-        if (st != NK_OK) return st;
+        if (e != cudaSuccess) { what = "nk_helmholtz_apply_host: H2D"; break; }
+        st = run_op(nk::OP_HELM, "nk_helmholtz_apply_host", b, g, 0, g->d_stage_in, nullptr, nullptr, g->d_stage_out,
+                    nullptr, nullptr, lambda, stream, 1, nullptr, nullptr, g0, g1 - g0);
+        if (st != NK_OK) break;
         e = cudaEventRecord(g->ev_k[c], s);
         if (e == cudaSuccess) e = cudaStreamWaitEvent(g->s_out, g->ev_k[c], 0);
         if (e == cudaSuccess) e = cudaMemcpyAsync(host_out + off, g->d_stage_out + off, nb, cudaMemcpyDeviceToHost, g->s_out);
-        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: D2H");
+        if (e != cudaSuccess) { what = "nk_helmholtz_apply_host: D2H"; break; }
+    }
+    if (e != cudaSuccess || st != NK_OK) {
+        // drain everything that was enqueued: no copy into host_out may still be in flight when we return
+        const std::string keep = g_err;
+        cudaStreamSynchronize(g->s_in);
+        cudaStreamSynchronize(s);
+        cudaStreamSynchronize(g->s_out);
+        if (st != NK_OK) { g_err = keep; return st; }
+        return cuda_fail(e, what ? what : "nk_helmholtz_apply_host");
     }
     e = cudaEventRecord(g->ev_done, g->s_out);
     if (e == cudaSuccess) e = cudaStreamWaitEvent(s, g->ev_done, 0);
     if (e == cudaSuccess) e = cudaStreamSynchronize(s);
-    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_host: synchronise");
+    if (e != cudaSuccess) {
+        cudaStreamSynchronize(g->s_in);
+        cudaStreamSynchronize(g->s_out);
+        return cuda_fail(e, "nk_helmholtz_apply_host: synchronise");
+    }
     return NK_OK;
 }
 

@@ -3,6 +3,7 @@
 // deformed, op) replaces the paper's JIT (north_star).
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 
 #include "nk_kernel_body.cuh"
 #include "nk_launch.h"
@@ -17,7 +18,16 @@ template <int SHAPE, int P, int DEF, int OP>
 static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const KArgs& a, int num_sms, cudaStream_t stream)
 {
     using T = TuneOp<SHAPE, P, DEF, OP>;
-    static int blocks_per_sm = 0;
+    // function attributes and occupancy are per device: one cache entry per device ordinal, filled under a lock
+    enum { kMaxDevices = 64 };
+    static int bps_cache[kMaxDevices] = {};
+    static std::mutex mu;
+    int dev = 0;
+    {
+        cudaError_t de = cudaGetDevice(&dev);
+        if (de != cudaSuccess) return de;
+        if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+    }
     DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs;
     std::memcpy(&tabs, tabs_flat, sizeof(tabs));
     typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st;
@@ -28,7 +38,10 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
     static_assert(sizeof(tabs) + sizeof(st) + sizeof(KArgs) <= 32000, "kernel parameters exceed the 32 KB limit");
     const size_t smem = T::smem_grid;
     auto kern = nk_kernel<SHAPE, P, DEF, OP>;
-    if (blocks_per_sm == 0) {
+    int blocks_per_sm;
+    {
+    std::lock_guard<std::mutex> lk(mu);
+    if (bps_cache[dev] == 0) {
         cudaError_t err = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
         if (err != cudaSuccess) return err;
         err = cudaFuncSetAttribute(kern, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared);
@@ -36,21 +49,22 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
         int bps = 0;
         err = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&bps, kern, T::NT, smem);
         if (err != cudaSuccess) return err;
-        blocks_per_sm = bps < 1 ? 1 : bps;
+        bps_cache[dev] = bps < 1 ? 1 : bps;
+    }
+    blocks_per_sm = bps_cache[dev];
     }
     if (a.grid_groups <= 0) return cudaSuccess;
     KArgs b = a;
     // L2 prefetch distance = 1/8 of the co-resident blocks (B200 sweep, profiles/r1_notes.md: flat between 3 %
     // and 25 %; at 100 % a third of the prefetched lines are evicted before use and re-read from DRAM).
     // NK_PREFETCH_PCT rescales it (percent of the co-resident blocks; 0 = off).
-    static int pf_pct = -1;
-    if (pf_pct < 0) {
+    static const int pf_pct = [] {
         const char* ev = std::getenv("NK_PREFETCH_PCT");
-        pf_pct = ev ? std::atoi(ev) : 12;
-    }
-    b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * T::WPB * pf_pct / 100) + 1 : 0x3fffffff;
+        return ev ? std::atoi(ev) : 12;
+    }();
+    b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * pf_pct / 100) + 1 : 0x3fffffff;
     const long long units = (long long)a.grid_groups * (a.nfields > 1 ? a.nfields : 1);   // (group, field) pairs
-    const long long nblocks = (units + T::WPB - 1) / T::WPB;                               // WPB of them per block in WP mode
+    const long long nblocks = units;
     if (nblocks > 0x7fffffffLL) return cudaErrorInvalidConfiguration;
     kern<<<(unsigned)nblocks, T::NT, smem, stream>>>(tabs, st, b);
     return cudaGetLastError();

@@ -71,24 +71,17 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
     constexpr bool KRON = T::KRON;
     constexpr int EG = Tune<SHAPE, P, DEF>::E;         // interleave width of the geometry stream
 
-    constexpr bool WP = T::WP;
     extern __shared__ double sm[];
-    // block-wide variant: thread = (e, slot) over the whole block; WP variant: the same within each warp,
-    // which owns its own X, Y, Z slice and its own group of E elements
-    const int tid = WP ? (int)(threadIdx.x & 31) : (int)threadIdx.x;
-    const int wgrp = WP ? (int)(threadIdx.x >> 5) : 0;
+    // thread = (e, slot) over the whole block
+    const int tid = (int)threadIdx.x;
     // general path: X, Y, Z; coefficient-space kernels: Y, Z, X(, fourth array) in that order (see their .inc)
-    double* __restrict__ S0 = sm + (size_t)wgrp * 3 * NQP * E;
+    double* __restrict__ S0 = sm;
     double* __restrict__ X = S0 + (size_t)(T::KRON ? 2 : 0) * NQP * E;
     double* __restrict__ Y = S0 + (size_t)(T::KRON ? 0 : 1) * NQP * E;
     double* __restrict__ Z = S0 + (size_t)(T::KRON ? 1 : 2) * NQP * E;
     const int e = tid % E, slot = tid / E;
-    const bool active = !WP || tid < E * LS;     // WP: lanes beyond E*Q^2 (27 of 32 at Q = 3, 25 at Q = 5) idle
-#define NK_SYNC()                                   \
-    do {                                            \
-        if constexpr (WP) __syncwarp();             \
-        else __syncthreads();                       \
-    } while (0)
+    constexpr bool active = true;
+#define NK_SYNC() __syncthreads()
 #define GIDX(i, j, k) (((i) + LQ * ((j) + Q * (k))) * E + e)
 // partial transforms T1[l][k] (after the r-sum) and T2[p][j][k] (after the q-sum): the k-stride LQ is odd
 // when E < 16, so that threads on consecutive lines l or j fall into different banks
@@ -105,12 +98,9 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
     // spills per thread and a third of the issue slots lost).
     {
         constexpr bool FIELDS = (OPX == OP_HELMF);
-        const long long unit = WP ? (long long)blockIdx.x * T::WPB + wgrp : (long long)blockIdx.x;   // group x field
+        const long long unit = (long long)blockIdx.x;   // group x field
         const int fld = (FIELDS && a.nfields > 1) ? (int)(unit % a.nfields) : 0;
         const int g = a.g0 + ((FIELDS && a.nfields > 1) ? (int)(unit / a.nfields) : (int)unit);
-        if constexpr (WP) {
-            if (g >= a.g0 + a.grid_groups) return;      // surplus warps of the last block (no block barrier in WP mode)
-        }
         // field pointers are re-read from the parameter bank where they are used (no registers held across stages)
 #define NK_FIN0 (FIELDS ? a.fin[fld] : a.in[0])
 #define NK_FOUT0 (FIELDS ? a.fout[fld] : a.out[0])
@@ -130,7 +120,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
             // the same for the next group's input fields (element-major, contiguous per group)
             constexpr int NIN = IN_COEFF ? NMODES : NQ;
             const int gn = g + a.pf_dist;
-            if (gn < a.ngroups && tid == (WP ? 0 : 32)) {
+            if (gn < a.ngroups && tid == 32) {
                 const double* base = IN_COEFF ? NK_FIN0 : a.in[0];
                 if (base && (reinterpret_cast<size_t>(base) & 15) == 0) {
                     const long long e0 = (long long)gn * E;

@@ -44,28 +44,13 @@ __host__ __device__ constexpr int k_num_modes(int shape, int nm)
 // Values from the round-1 sweeps on B200 (profiles/r1_notes.md): deformed (HBM-bound) kernels want small
 // blocks (about 150-200 threads) at up to 96 registers, many of them per SM; affine (issue / shared-memory
 // bound) kernels want 72 registers and as many resident threads as that allows.
-//
-// WP ("warp-private" elements; the low-order variant, cf. the paper's threading over elements): at
-// Q <= 5 all Q^2 lines of 32/Q^2 elements fit ONE warp.  Each warp then owns its elements and its own slice
-// of shared memory, and the stages are separated by __syncwarp() instead of block barriers, which dominate the
-// run time when a stage is only 9..25 short lines.  Hexes only.  MEASURED SLOWER on B200 and therefore OFF by
-// default (build with -DNK_TUNE_WP=1 to try it): config 4 mass + Laplacian P1 22.0 vs 30.8, P2 37.4 vs 45.7,
-// P3 36.7 vs 40.5 GDoF/s -- the block barriers are not what limits the low orders; the idle lanes (27 or 25 of
-// 32) and the bank conflicts of a 2-3 element interleave cost more than the barriers save.
 template <int SHAPE, int P, int DEF>
 struct Tune {
     static constexpr int Q = P + 2;
-#if defined(NK_TUNE_WP)
-    static constexpr bool WP = (NK_TUNE_WP != 0) && SHAPE == K_HEX && Q <= 5;
-#else
-    static constexpr bool WP = false;
-#endif
-    static constexpr int WPB = WP ? 8 : 1;          // warps (= independent groups) per block in WP mode
 #if defined(NK_TUNE_E)
-    static constexpr int E = WP ? 32 / (Q * Q) : NK_TUNE_E;
+    static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = WP ? 32 / (Q * Q)
-                             : DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : 4)
+    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : 4)
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
@@ -92,8 +77,8 @@ struct Tune {
     // used once (nothing for the compiler to hoist and spill)
     static constexpr int LS = SHAPE == K_HEX ? Q * Q : cdiv((Q * Q > LS_min ? Q * Q : LS_min), SPW) * SPW;
 #endif
-    static constexpr int NT = WP ? 32 * WPB : E * LS;
-    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double) * WPB;
+    static constexpr int NT = E * LS;
+    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
@@ -110,7 +95,7 @@ struct Tune {
 template <int SHAPE, int P, int DEF, int OPX>
 struct TuneOp : Tune<SHAPE, P, DEF> {
     using B = Tune<SHAPE, P, DEF>;
-    static constexpr bool AFF_HEX = (SHAPE == K_HEX && !DEF && !B::WP);
+    static constexpr bool AFF_HEX = (SHAPE == K_HEX && !DEF);
     static constexpr bool MASS_KRON = AFF_HEX && OPX == OP_MASS;                                   // nk_stage_masskron.inc
 #if defined(NK_NO_LAPKRON)
     static constexpr bool LAP_KRON = false;

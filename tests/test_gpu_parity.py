@@ -264,7 +264,7 @@ def test_helmholtz_host_entry(nk, deformed):
     y = torch.empty_like(x).pin_memory()
     n0 = nk.launch_count()
     nk.helmholtz_apply_host(basis, geom, 1.0, x, y)
-    assert 1 <= nk.launch_count() - n0 <= 8      # chunked copy / compute / copy pipeline
+    assert 1 <= nk.launch_count() - n0 <= 16     # chunked copy / compute / copy pipeline
     ref = o.helmholtz(el, A.numpy(), J.numpy(), 1.0, x.numpy())
     assert K.normwise_err(y.numpy(), ref) <= TOL
 
