@@ -177,6 +177,10 @@ nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, double* host_o
 /* Register-only DFMA chains on every SM for `iters` x 1024 FMAs per thread (8 independent chains); *tflops receives the
  * sustained fp64 rate (2 flop per FMA).  This is the measured FP64 roofline denominator.            */
 nk_status nk_probe_fp64_peak(int iters, double* tflops, double* ms);
+/* The same on the FP64 tensor-core path: mma.sync m8n8k4 f64 (SASS DMMA.8x8x4), 8 independent accumulator chains per
+ * warp, `iters` x 128 DMMA per warp.  On B200 both probes read 37.05 TFLOP/s: DMMA and DFMA share one pipe with one
+ * peak; what DMMA saves is issue slots and operand traffic (8 FMA per lane and instruction).                        */
+nk_status nk_probe_fp64_dmma_peak(int iters, double* tflops, double* ms);
 /* number of kernels this library has launched from the calling process so far                      */
 int64_t nk_launch_count(void);
 const char* nk_last_error(void);

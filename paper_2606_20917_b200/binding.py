@@ -46,6 +46,7 @@ _SIG = {
     "nk_get_affine_simplex_form": (_i, []),
     "nk_basis_get_reference_matrix": (_i, [_p, _i, C.POINTER(_d), _sz]),
     "nk_probe_fp64_peak": (_i, [_i, C.POINTER(_d), C.POINTER(_d)]),
+    "nk_probe_fp64_dmma_peak": (_i, [_i, C.POINTER(_d), C.POINTER(_d)]),
     "nk_launch_count": (_i64, []),
     "nk_last_error": (C.c_char_p, []),
     "nk_version": (C.c_char_p, []),
@@ -287,6 +288,12 @@ def get_affine_simplex_form():
 def probe_fp64_peak(iters=200):
     tf, ms = _d(), _d()
     _check(lib.nk_probe_fp64_peak(iters, C.byref(tf), C.byref(ms)))
+    return tf.value, ms.value
+
+
+def probe_fp64_dmma_peak(iters=200):
+    tf, ms = _d(), _d()
+    _check(lib.nk_probe_fp64_dmma_peak(iters, C.byref(tf), C.byref(ms)))
     return tf.value, ms.value
 
 

@@ -808,6 +808,57 @@ extern "C" nk_status nk_probe_fp64_peak(int iters, double* tflops, double* ms_ou
     return NK_OK;
 }
 
+namespace {
+// the same for the FP64 tensor-core path: 8 independent DMMA.8x8x4 accumulator chains per warp, 128 DMMA per trip
+__global__ void __launch_bounds__(256) dmma_probe(int iters, double x, double y, double* sink)
+{
+    double acc[8][2];
+#pragma unroll
+    for (int c = 0; c < 8; ++c) { acc[c][0] = threadIdx.x * 1e-9 + c; acc[c][1] = c; }
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u)
+#pragma unroll
+            for (int c = 0; c < 8; ++c) nk::dmma884(acc[c][0], acc[c][1], x, y);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int c = 0; c < 8; ++c) s += acc[c][0] + acc[c][1];
+    if (s == 123.456) sink[0] = s;
+}
+} // namespace
+
+extern "C" nk_status nk_probe_fp64_dmma_peak(int iters, double* tflops, double* ms_out)
+{
+    if (iters < 1 || !tflops) return fail(NK_ERR_INVALID_ARG, "nk_probe_fp64_dmma_peak: bad arguments");
+    nk_status st = ensure_device();
+    if (st != NK_OK) return st;
+    double* sink = nullptr;
+    cudaError_t e = cudaMalloc(&sink, sizeof(double));
+    if (e != cudaSuccess) return cuda_fail(e, "nk_probe_fp64_dmma_peak: cudaMalloc");
+    cudaEvent_t t0, t1;
+    cudaEventCreate(&t0);
+    cudaEventCreate(&t1);
+    const int blocks = g_num_sms * 8, threads = 256;
+    dmma_probe<<<blocks, threads>>>(1, 0.999999, 1e-9, sink); // warm-up
+    cudaEventRecord(t0);
+    dmma_probe<<<blocks, threads>>>(iters, 0.999999, 1e-9, sink);
+    cudaEventRecord(t1);
+    e = cudaEventSynchronize(t1);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, t0, t1);
+    cudaEventDestroy(t0);
+    cudaEventDestroy(t1);
+    cudaFree(sink);
+    { std::lock_guard<std::mutex> lk(g_mutex); g_launches += 2; }
+    if (e != cudaSuccess) return cuda_fail(e, "nk_probe_fp64_dmma_peak");
+    // one m8n8k4 DMMA = 8 x 8 x 4 FMA per warp
+    const double flops = 2.0 * 256.0 * 128.0 * iters * (double)blocks * (threads / 32);
+    *tflops = flops / (ms * 1e-3) / 1e12;
+    if (ms_out) *ms_out = ms;
+    return NK_OK;
+}
+
 extern "C" int64_t nk_launch_count(void)
 {
     std::lock_guard<std::mutex> lk(g_mutex);
