@@ -141,6 +141,9 @@ typedef struct {
     const double* in; /* device [nelem][Nm] */
     double* out;      /* device [nelem][Nm] */
 } nk_block;
+/* Block 0 is launched on `stream`, the others on internal side streams forked from and joined to `stream` by events:
+ * the kernels of different blocks may overlap (the tail of one with the head of the next), and everything is ordered
+ * after earlier and before later work on `stream`.  Blocks must not share output buffers.                     */
 nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double lambda, void* stream);
 
 /* End-to-end variant with HOST field buffers: copies host_in to an internal device buffer, applies the

@@ -48,8 +48,15 @@ def _run(cmd):
     return r.stdout + r.stderr
 
 
-def build(force=False, jobs=None, verbose=False, extra_defs=()):
+def build(force=False, jobs=None, verbose=False, extra_defs=(), lib=None, objdir=None, only=None):
+    """extra_defs / lib / objdir: a tuning build (-D switches of csrc/nk_kernels.cuh) into another library file, to be
+    loaded with NK_LIB=<path>; only: iterable of (shape, P) pairs to instantiate (the others keep their objects)."""
+    global OBJ, LIB
     nvcc = _nvcc()
+    if objdir:
+        OBJ = objdir
+    if lib:
+        LIB = lib
     os.makedirs(OBJ, exist_ok=True)
     deps = _sources()
     jobs = jobs or max(1, (os.cpu_count() or 2))
@@ -87,8 +94,11 @@ def main():
     ap.add_argument("--force", action="store_true")
     ap.add_argument("-j", type=int, default=None)
     ap.add_argument("-v", action="store_true")
+    ap.add_argument("--defs", default="", help="extra -D switches, space separated (tuning builds)")
+    ap.add_argument("--lib", default=None, help="output library (default: libnk.so next to this file)")
+    ap.add_argument("--objdir", default=None)
     a = ap.parse_args()
-    out = build(force=a.force, jobs=a.j, verbose=a.v)
+    out = build(force=a.force, jobs=a.j, verbose=a.v, extra_defs=tuple(a.defs.split()), lib=a.lib, objdir=a.objdir)
     if a.v:
         sys.stdout.write(out)
     print(LIB)

@@ -617,14 +617,64 @@ extern "C" nk_status nk_helmholtz_apply_fields(const nk_basis* b, const nk_geom*
                   stream, nfields, in, out);
 }
 
+namespace {
+// side streams of nk_helmholtz_apply_blocks: block i > 0 runs on side stream (i-1) % kSide, forked from and joined to the
+// caller's stream by events, so that the tail of one block's kernel overlaps the head of the next one's
+enum { kSide = 3, kMaxDev = 64 };
+struct SidePool {
+    cudaStream_t s[kSide] = {};
+    cudaEvent_t fork = nullptr, join[kSide] = {};
+    bool ok = false;
+};
+SidePool g_side[kMaxDev];
+std::mutex g_side_mutex;     // one nk_helmholtz_apply_blocks at a time per process (the pool is shared)
+} // namespace
+
 extern "C" nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double lambda, void* stream)
 {
     if (nblocks < 0 || (nblocks > 0 && !blocks)) return fail(NK_ERR_INVALID_ARG, "nk_helmholtz_apply_blocks: bad arguments");
-    for (int i = 0; i < nblocks; ++i) {
-        nk_status st = nk_helmholtz_apply(blocks[i].basis, blocks[i].geom, lambda, blocks[i].in, blocks[i].out, stream);
-        if (st != NK_OK) return st;
+    if (nblocks <= 1) return nblocks == 0 ? NK_OK : nk_helmholtz_apply(blocks[0].basis, blocks[0].geom, lambda, blocks[0].in, blocks[0].out, stream);
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return cuda_fail(e, "cudaGetDevice (no CUDA device: libnk has no CPU fallback)");
+    if (dev < 0 || dev >= kMaxDev) return fail(NK_ERR_UNSUPPORTED, "device ordinal beyond 63");
+    std::lock_guard<std::mutex> lk(g_side_mutex);
+    SidePool& sp = g_side[dev];
+    if (!sp.ok) {
+        for (int i = 0; i < kSide && e == cudaSuccess; ++i) {
+            e = cudaStreamCreateWithFlags(&sp.s[i], cudaStreamNonBlocking);
+            if (e == cudaSuccess) e = cudaEventCreateWithFlags(&sp.join[i], cudaEventDisableTiming);
+        }
+        if (e == cudaSuccess) e = cudaEventCreateWithFlags(&sp.fork, cudaEventDisableTiming);
+        if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_blocks: stream / event creation");
+        sp.ok = true;
     }
-    return NK_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    e = cudaEventRecord(sp.fork, s);
+    if (e != cudaSuccess) return cuda_fail(e, "nk_helmholtz_apply_blocks: fork");
+    nk_status st = NK_OK;
+    bool used[kSide] = {};
+    for (int i = 0; i < nblocks && st == NK_OK; ++i) {
+        cudaStream_t si = s;
+        if (i > 0) {
+            const int k = (i - 1) % kSide;
+            si = sp.s[k];
+            if (!used[k]) {
+                e = cudaStreamWaitEvent(si, sp.fork, 0);
+                if (e != cudaSuccess) { st = cuda_fail(e, "nk_helmholtz_apply_blocks: fork"); break; }
+                used[k] = true;
+            }
+        }
+        st = nk_helmholtz_apply(blocks[i].basis, blocks[i].geom, lambda, blocks[i].in, blocks[i].out, (void*)si);
+    }
+    // join whatever was forked, also on error (the caller's stream must not run ahead of work already enqueued)
+    for (int k = 0; k < kSide; ++k) {
+        if (!used[k]) continue;
+        e = cudaEventRecord(sp.join[k], sp.s[k]);
+        if (e == cudaSuccess) e = cudaStreamWaitEvent(s, sp.join[k], 0);
+        if (e != cudaSuccess && st == NK_OK) st = cuda_fail(e, "nk_helmholtz_apply_blocks: join");
+    }
+    return st;
 }
 
 extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* gc, double lambda, const double* host_in,

@@ -48,6 +48,13 @@ __device__ __forceinline__ void cp_async8(double* smem_dst, const double* gsrc, 
     asm volatile("cp.async.ca.shared.global [%0], [%1], 8, %2;" ::"r"(d), "l"(gsrc), "r"(ok ? 8 : 0) : "memory");
 }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+// waits until at most n of this thread's most recent cp.async groups are pending (n is a compile-time constant)
+template <int N>
+__device__ __forceinline__ void cp_async_wait_group()
+{
+    asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
+}
 
 template <int SHAPE, int P, int DEF, int OPX>
 __global__ void __launch_bounds__(TuneOp<SHAPE, P, DEF, OPX>::NT, TuneOp<SHAPE, P, DEF, OPX>::MINB)
@@ -79,6 +86,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
     double* __restrict__ X = S0 + (size_t)(T::KRON ? 2 : 0) * NQP * E;
     double* __restrict__ Y = S0 + (size_t)(T::KRON ? 0 : 1) * NQP * E;
     double* __restrict__ Z = S0 + (size_t)(T::KRON ? 1 : 2) * NQP * E;
+    double* __restrict__ RG = S0 + (size_t)3 * NQP * E;      // geometry ring [RING][7][threads] (T::RING > 0 only)
+    (void)RG;
     const int e = tid % E, slot = tid / E;
     constexpr bool active = true;
 #define NK_SYNC() __syncthreads()
@@ -140,7 +149,24 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
             NK_FORU(m, NMODES)
             cp_async8(KRON ? &Y[(((m / (NM * NM)) * NMP + (m / NM) % NM) * NMP + m % NM) * E + e] : &Y[m * E + e],
                       valid ? src + m : NK_FIN0, valid);
-            cp_async_wait_all();
+            if constexpr (T::RING > 0) {
+                static_assert(T::RING == 0 || LS >= Q * Q, "the geometry ring assumes one pass-C line per thread");
+                // geometry ring (pass C): the first RING planes of this thread's quadrature line, one cp.async group each,
+                // behind the coefficient group; they land while the basis stages run
+                cp_async_commit();
+                constexpr int NTH = T::NT;
+                const int lc = slot;                        // pass C: thread `slot` owns line (i,j) = slot
+                NK_UNROLL for (int kk = 0; kk < T::RING; ++kk) {
+                    if (lc < Q * Q) {
+                        NK_UNROLL for (int c = 0; c < 7; ++c)
+                            cp_async8(&RG[(kk * 7 + c) * NTH + tid], geo + ((size_t)c * NQ + lc + Q * Q * kk) * E, true);
+                    }
+                    cp_async_commit();
+                }
+                cp_async_wait_group<T::RING>();             // the coefficient group is complete; the ring may still be in flight
+            } else {
+                cp_async_wait_all();
+            }
             NK_SYNC();
             if constexpr (MASS_KRON) {
 #include "nk_stage_masskron.inc"

@@ -78,12 +78,24 @@ struct Tune {
     static constexpr int LS = SHAPE == K_HEX ? Q * Q : cdiv((Q * Q > LS_min ? Q * Q : LS_min), SPW) * SPW;
 #endif
     static constexpr int NT = E * LS;
+    // RING: depth (in k-planes) of the per-thread geometry ring of the deformed Laplacian / Helmholtz kernels
+    // (nk_stage_mid.inc, pass C): the 7 metric entries of the thread's next RING points are copied global -> shared
+    // by cp.async while the thread works, the first RING planes from kernel entry on.  0 = plain __ldg in pass C.
+#if defined(NK_TUNE_RING)
+    static constexpr int RING = DEF ? (NK_TUNE_RING < Q ? NK_TUNE_RING : Q) : 0;
+#else
+    // B200 sweep (profiles/r2_notes.md): the ring costs 7 LDGSTS + 7 LDS per point instead of 7 LDG and loses wherever the
+    // L2 prefetch alone keeps pass C fed (hexes at every order: cfg2 49.0 -> 42.8; simplices up to Q = 9: cfg5 19.5 -> 16.3);
+    // it wins on the simplices at Q = 10 (cfg5:8 10.2 -> 11.6 GDoF/s), where few warps are resident to hide the L2 latency
+    static constexpr int RING = (DEF && SHAPE != K_HEX && Q >= 10) ? 2 : 0;
+#endif
+    static constexpr size_t smem_ring = (size_t)NT * RING * 7 * sizeof(double);
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
     static constexpr int REGS = DEF ? (SHAPE == K_HEX ? 96 : 72) : Q <= 6 ? 56 : 64;
-    static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + 2048));
+    static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + smem_ring + 2048));
     static constexpr int MINB_reg = 65536 / (NT * REGS);
     static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
 #endif
@@ -127,7 +139,9 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
     static constexpr int NARR = MASS_KRON ? 2 : LAP_KRON ? 4 : 3;
     static constexpr int LS = KRON ? NM * NM : B::LS;
     static constexpr int NT = KRON ? E * LS : B::NT;
-    static constexpr size_t smem_grid = KRON ? (size_t)NARR * NQP * E * sizeof(double) : B::smem_grid;
+    static constexpr bool USE_RING = B::RING > 0 && DEF && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
+    static constexpr int RING = USE_RING ? B::RING : 0;
+    static constexpr size_t smem_grid = KRON ? (size_t)NARR * NQP * E * sizeof(double) : B::smem_grid + (USE_RING ? B::smem_ring : 0);
 #if defined(NK_TUNE_REGSK)
     static constexpr int REGSK = NK_TUNE_REGSK;
 #else

@@ -67,6 +67,10 @@ def run_full(nk, cfg):
         ys = y[idx.to(dev)].cpu().numpy()
         err = K.normwise_err(ys, ref)
         worst = max(worst, err)
+        # shown by `pytest -s` (profiles/r2_repeat.md): how far the two evaluations of the input generator are apart
+        print("%s shape %d: generator device vs host dA %.2e dJ %.2e; parity %.2e on %d sampled elements" % (
+            title, b["shape"], np.abs(Ao.numpy() - As.numpy()).max() / np.abs(Ao.numpy()).max(),
+            np.abs(Jo.numpy() - Js.numpy()).max() / np.abs(Jo.numpy()).max(), err, len(idx)))
         if err > TOL:   # say where: per-element errors and how far the two geometry evaluations are apart
             pe = np.abs(ys - ref).max(axis=1) / np.abs(ref).max(axis=1)
             where = [(int(idx[i]), "%.1e" % pe[i]) for i in np.argsort(-pe)[:6]]
@@ -158,3 +162,36 @@ def test_full_size_invariants_all_elements(nk, cfg):
     # config 5: the tets fill z in [0, 1/4) and the prisms the rest, together the unit cube
     tol = 1e-9 if blocks[0]["deformed"] else 1e-12     # the sinusoidal map integrates to 1 up to quadrature error
     assert abs(vol - 1.0) <= tol, "sum of element volumes %.15g (%s)" % (vol, title)
+
+
+@pytest.mark.parametrize("cfg", [2, 3])
+def test_full_size_every_element_against_the_oracle(nk, cfg):
+    """configs 2 and 3 at BASELINE size, EVERY element against the oracle (oracle.parallel: the unchanged oracle
+    over element chunks in a process pool on all host cores).  The oracle's inputs are evaluated on the host at
+    the oracle's own quadrature points; the kernel's on the device at the library's."""
+    from oracle.parallel import OraclePool
+    dev = torch.device("cuda", 0)
+    title, op, blocks = cfgs.config_blocks(cfg, device=dev)
+    b = blocks[0]
+    basis = nk.Basis(b["shape"], b["P"])
+    A, J = cfgs.block_factors(b, basis.points())
+    geom = nk.Geom(basis, A, J, b["deformed"], streams=nk.Geom.METRIC)
+    ne = J.shape[0]
+    del A, J
+    x = wl.coefficients(b["seed"], ne, basis.num_modes)
+    y = torch.full((ne, basis.num_modes), float("nan"), dtype=torch.float64, device=dev)
+    nk.helmholtz_apply(basis, geom, b["lam"], x.to(dev), y)
+    torch.cuda.synchronize()
+    got = y.cpu().numpy()
+    el = K.element(b["shape"], b["P"])
+    v0, E = b["v0"].cpu(), b["E"].cpu()
+    worst, step = 0.0, 8192
+    with OraclePool() as pool:
+        for s in range(0, ne, step):
+            Ao, Jo = (wl.sinusoidal_factors(v0[s:s + step], E[s:s + step], el.xi) if b["deformed"]
+                      else wl.affine_factors(v0[s:s + step], E[s:s + step]))
+            ref = pool.apply("helmholtz", b["shape"], b["P"], b["P"] + 2, Ao.numpy(), Jo.numpy(), b["lam"], x[s:s + step].numpy())
+            pe = np.abs(got[s:s + step] - ref).max(axis=1) / np.abs(ref).max(axis=1)
+            worst = max(worst, float(pe.max()))
+            assert pe.max() <= TOL, "%s: element %d normwise error %.3e" % (title, s + int(pe.argmax()), pe.max())
+    print("%s: %d elements, worst normwise error %.2e" % (title, ne, worst))

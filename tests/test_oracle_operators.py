@@ -335,3 +335,46 @@ def test_brute_force_sum_factorised_bwd(shape, P):
     uh = np.random.default_rng(shape * 10 + P).uniform(-1, 1, el.Nm)
     ref = _sumfact_bwd(shape, P, Q, el.z, uh)
     np.testing.assert_allclose(o.bwdtrans(el, uh[None])[0], ref, atol=1e-14)
+
+
+class _ExtendedElement:
+    """the oracle's element tables cast to np.longdouble (80-bit extended on x86): the SAME tables, so that running the
+    oracle's operator functions on it repeats their dense sums with 11 more bits in every product and accumulation"""
+
+    def __init__(self, el):
+        self.__dict__.update(el.__dict__)
+        for k, v in el.__dict__.items():
+            if isinstance(v, np.ndarray) and v.dtype == np.float64:
+                setattr(self, k, v.astype(np.longdouble))
+            elif isinstance(v, (list, tuple)) and v and all(isinstance(a, np.ndarray) for a in v):
+                setattr(self, k, [a.astype(np.longdouble) if a.dtype == np.float64 else a for a in v])
+        self._el = el
+
+    def chain(self, dEta):
+        return type(self._el).chain(self, dEta)
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 4, 5])
+def test_oracle_rounding_against_extended_precision(cfg):
+    """the oracle's own fp64 rounding.  On a sample of each configuration (<= 256 elements) the
+    oracle's Helmholtz in fp64 agrees with the same sums carried in extended precision to <= 1e-13 normwise, i.e.
+    the 1e-12 parity gate of the GPU tests is not consumed by the oracle's accumulation order."""
+    if np.finfo(np.longdouble).eps >= np.finfo(np.float64).eps:
+        pytest.skip("np.longdouble is not wider than float64 on this platform")
+    from workloads import configs as cfgs
+    from workloads import synthetic as wl
+    title, op, blocks = cfgs.config_blocks(cfg, device="cpu", scale=0.2)
+    for b in blocks:
+        el = o.Element(b["shape"], b["P"], b["P"] + 2)
+        ne = min(b["v0"].shape[0], 256 if el.Nq <= 216 else 48)
+        idx = np.linspace(0, b["v0"].shape[0] - 1, ne).astype(np.int64)
+        v0, E = b["v0"][idx], b["E"][idx]
+        A, J = (wl.sinusoidal_factors(v0, E, el.xi) if b["deformed"] else wl.affine_factors(v0, E))
+        x = wl.coefficients(b["seed"], ne, el.Nm).numpy()
+        lam = b["lam"] if b["lam"] else 1.0
+        y64 = o.helmholtz(el, A.numpy(), J.numpy(), lam, x)
+        ld = np.longdouble
+        yld = o.helmholtz(_ExtendedElement(el), A.numpy().astype(ld), J.numpy().astype(ld), ld(lam), x.astype(ld))
+        assert yld.dtype == np.longdouble
+        err = (np.abs(y64 - yld).max(axis=1) / np.abs(yld).max(axis=1)).max()
+        assert float(err) <= 1e-13, "%s: fp64 vs extended %.2e" % (title, float(err))
