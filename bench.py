@@ -24,7 +24,7 @@ METRIC = "Helmholtz apply GDoF/s (fp64)"
 HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SM x 64 DFMA/clk x 2 x 1.965 GHz
 PER_WORKLOAD_DEFAULT = ("cfg3", "cfg3:7", "cfg3:8", "cfg5", "cfg5:8", "cfg4:1", "cfg4:4", "cfg4:7", "cfg4:10",
-                        "cfg2:7", "cfg2:10", "cfg1")
+                        "cfg2:7", "cfg2:10", "cfg1", "cg")
 
 
 def parse_args():
@@ -304,10 +304,47 @@ def fractions(alg, ms, hbm_peak, fp64_tf):
     return {"bound": bound, "frac": hbm if bound == "hbm" else fp, "hbm_frac": hbm, "fp64_frac": fp, "fp64_frac_running_form": fpr}
 
 
+def measure_cg(nk, dev, barrier):
+    """the assembled Helmholtz system of config 2's mesh (32^3 deformed hexes, P4, lambda = 1, C0
+    connectivity of workloads.assembly) solved by Jacobi-preconditioned CG to 1e-8; time per iteration (gather + fused
+    elemental kernel + scatter + 3 dot products + 3 vector updates) and the assembled apply on its own."""
+    import torch
+    from workloads import assembly as asm
+    from workloads import synthetic as wl
+    n, P, lam = 32, 4, 1.0
+    basis = nk.Basis(0, P)
+    v0, E = wl.hex_mesh(n, device=dev)
+    A, J = wl.sinusoidal_factors(v0, E, basis.points().to(dev))
+    geom = nk.Geom(basis, A, J, True, streams=nk.Geom.METRIC)
+    del A, J
+    l2g, ng = asm.hex_l2g(n, P)
+    gs = nk.GatherScatter(l2g, ng)
+    b = wl.coefficients(5, 1, ng).reshape(ng).to(dev)
+    x = torch.zeros_like(b)
+    nk.cg_solve(basis, geom, gs, lam, b, x, rtol=0.5, maxit=2)      # warm-up: builds the diagonal
+    x.zero_()
+    barrier()
+    t0 = time.perf_counter()
+    iters, rel = nk.cg_solve(basis, geom, gs, lam, b, x, rtol=1e-8, maxit=5000)
+    barrier()
+    dt = time.perf_counter() - t0
+    y = torch.empty_like(b)
+    ms_apply = timed(lambda i: nk.assembled_helmholtz_apply(basis, geom, gs, lam, b, y), 50, 3, barrier)
+    out = {"workload": "CG on the assembled system of 32^3 deformed hexes P4 (%d global dofs, %d local)" % (ng, l2g.numel()),
+           "iterations": iters, "relative_residual": rel, "ms_total": dt * 1e3, "ms_per_iteration": dt * 1e3 / max(iters, 1),
+           "assembled_apply_ms": ms_apply, "assembled_apply_gdofs": ng / (ms_apply * 1e-3) / 1e9,
+           "note": "wall clock around nk_cg_solve (it synchronises once per iteration to read the residual norm)"}
+    del gs, geom
+    torch.cuda.empty_cache()
+    return out
+
+
 def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budget_ms=400.0):
     """One entry of roofline.per_workload: the workload timed with the protocol of the headline (CUDA events, >= 3
     warm-ups, rotating buffers), about `budget_ms` of kernel time."""
     import torch
+    if name == "cg":
+        return measure_cg(nk, dev, barrier)
     w = Workload(nk, name, dev, rank)
     ms0 = timed(w.step, 3, 3, barrier)
     steps = int(max(10, min(2000, budget_ms / max(ms0, 1e-4))))

@@ -158,6 +158,41 @@ nk_status nk_helmholtz_apply_blocks(int nblocks, const nk_block* blocks, double 
 nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g, double lambda, const double* host_in,
                                   double* host_out, void* stream);
 
+/* ---- assembly and solver ---------------------------------------------------
+ * The paper leaves global assembly out and names the consumer of the elemental operators: "operator evaluations
+ * are required within the solver as part of a conjugate gradient or GMRES iteration".  A C0 expansion shares
+ * its vertex / edge / face modes between neighbouring elements: (Q u)[e][m] = sign[e][m] * u[l2g[e][m]] gathers a
+ * global vector into element-major local coefficients, Q^T adds local contributions into the global vector, and
+ * the assembled Helmholtz operator is A = Q^T diag(L^e + lambda M^e) Q (Eq. 6).  The map is the caller's
+ * (mesh connectivity is not part of this library).
+ * l2g: HOST [nelem][nm_local] global dof of every local mode, 0 <= l2g < nglobal; sign: HOST [nelem][nm_local] of +1 / -1
+ * (orientation of shared edge / face modes) or NULL for all +1.  Needs a CUDA device (the map lives on the device). */
+typedef struct nk_gs nk_gs;
+nk_status nk_gs_create(int64_t nelem, int nm_local, int64_t nglobal, const int64_t* l2g, const signed char* sign, nk_gs** out);
+nk_status nk_gs_destroy(nk_gs* gs);
+int64_t nk_gs_num_global(const nk_gs* gs);
+/* local = Q global: device [nglobal] -> device [nelem][nm_local]                                                  */
+nk_status nk_gs_gather(const nk_gs* gs, const double* global, double* local, void* stream);
+/* global = Q^T local (overwrites global).  Deterministic: one thread per global dof sums its local copies in the
+ * order of their local index (transposed map built by nk_gs_create); no atomics.                                  */
+nk_status nk_gs_scatter_add(const nk_gs* gs, const double* local, double* global, void* stream);
+/* out = Q^T (L + lambda M) Q in on device vectors [nglobal]: gather, ONE fused elemental kernel, scatter.          */
+nk_status nk_assembled_helmholtz_apply(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* in,
+                                       double* out, void* stream);
+/* Conjugate gradients on A x = rhs, A as above (symmetric positive definite for lambda > 0; no constrained dofs).
+ * precond: NK_PRECOND_NONE, or NK_PRECOND_JACOBI = diag(A)^-1 with diag(A) = Q^T diag(H^e); the elemental diagonals are
+ * obtained by applying the elemental operator to the Nm unit vectors (Nm launches, once per (geometry, lambda), cached in
+ * the nk_gs handle).  The modified basis is badly conditioned without it (16^3 deformed hexes at P4, lambda = 1, to
+ * 1e-8: 11384 iterations without, 705 with; profiles/r2_notes.md).
+ * x: initial guess on entry, solution on return (device [nglobal]); stops when ||r|| <= rtol ||rhs|| or after maxit
+ * iterations; *iters and *relres (may be NULL) receive the iteration count and the last ||r|| / ||rhs||.  All vector
+ * work runs on `stream`; the call synchronises it once per iteration to read the residual norm (8 bytes) and before
+ * returning.  Sums are reproducible run to run (fixed reduction grid).  Calls on one nk_gs are serialised by a lock
+ * in the handle (it owns the work vectors).                                                                        */
+enum { NK_PRECOND_NONE = 0, NK_PRECOND_JACOBI = 1 };
+nk_status nk_cg_solve(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* rhs, double* x,
+                      int precond, double rtol, int maxit, int* iters, double* relres, void* stream);
+
 /* ---- form of the affine simplex operators ------------------------------------------------------
  * With constant dxi/dx and |J| the operators of Eq. 6-7 are (L + lambda M)_e = sum_{c<6} G^e_c K_c +
  * lambda |J_e| K_6 with seven Nm x Nm matrices of the STANDARD element (the quadrature sums of Eq. 7 with the chain of

@@ -396,3 +396,27 @@ def element_matrices(el, dxi_dx, detJ):
     L = np.einsum("inm,n,inl->ml", gx, W, gx)
     return M, L
 
+
+
+# --------------------------------------------------------------------------
+# O4. Assembled operator (the paper leaves assembly out).
+# By definition the global matrix is the sum of the elemental matrices placed by
+# the local-to-global map: A = sum_e Q_e^T (L^e + lambda M^e) Q_e with
+# (Q_e)[m][g] = sign[e][m] if g == l2g[e][m] else 0.  Dense, tiny meshes only.
+# Pins (tests/test_oracle_operators.py): one element reproduces L^e + lambda M^e;
+# A is symmetric positive definite for lambda > 0; 1^T A 1 = lambda * volume and
+# L 1 = 0 (the vertex modes sum to 1); a global polynomial of degree <= P,
+# interpolated on the C0 modes, has the energy u^T A u of its exact integrals.
+# --------------------------------------------------------------------------
+def assembled_matrix(el, dxi_dx, detJ, lam, l2g, nglobal, sign=None):
+    """dense [nglobal][nglobal]; dxi_dx [ne][npt][3][3], detJ [ne][npt], l2g [ne][Nm] ints, sign [ne][Nm] of +-1."""
+    A = np.zeros((nglobal, nglobal))
+    for e in range(l2g.shape[0]):
+        M, L = element_matrices(el, dxi_dx[e], detJ[e])
+        H = L + lam * M
+        s = np.ones(el.Nm) if sign is None else sign[e].astype(np.float64)
+        H = s[:, None] * H * s[None, :]
+        for m in range(el.Nm):
+            for n in range(el.Nm):
+                A[l2g[e, m], l2g[e, n]] += H[m, n]
+    return A

@@ -42,6 +42,13 @@ _SIG = {
     "nk_helmholtz_apply_fields": (_i, [_p, _p, _d, _i, C.POINTER(_p), C.POINTER(_p), _p]),
     "nk_helmholtz_apply_blocks": (_i, [_i, _p, _d, _p]),
     "nk_helmholtz_apply_host": (_i, [_p, _p, _d, _p, _p, _p]),
+    "nk_gs_create": (_i, [_i64, _i, _i64, _p, _p, C.POINTER(_p)]),
+    "nk_gs_destroy": (_i, [_p]),
+    "nk_gs_num_global": (_i64, [_p]),
+    "nk_gs_gather": (_i, [_p, _p, _p, _p]),
+    "nk_gs_scatter_add": (_i, [_p, _p, _p, _p]),
+    "nk_assembled_helmholtz_apply": (_i, [_p, _p, _p, _d, _p, _p, _p]),
+    "nk_cg_solve": (_i, [_p, _p, _p, _d, _p, _p, _i, _d, _i, C.POINTER(_i), C.POINTER(_d), _p]),
     "nk_set_affine_simplex_form": (_i, [_i]),
     "nk_get_affine_simplex_form": (_i, []),
     "nk_basis_get_reference_matrix": (_i, [_p, _i, C.POINTER(_d), _sz]),
@@ -274,6 +281,55 @@ def helmholtz_apply_host(basis, geom, lam, host_in, host_out, stream=None):
     if host_in.numel() != n or host_out.numel() != n:
         raise ValueError("host buffers must hold nelem x Nm = %d values" % n)
     _check(lib.nk_helmholtz_apply_host(basis.h, geom.h, float(lam), _ptr(host_in), _ptr(host_out), _stream(stream)))
+
+
+class GatherScatter:
+    """nk_gs handle.  l2g: int64 CPU tensor [nelem][Nm]; sign: int8 CPU tensor of +-1 or None."""
+
+    def __init__(self, l2g, nglobal, sign=None):
+        if l2g.dtype != torch.int64 or l2g.is_cuda or not l2g.is_contiguous() or l2g.dim() != 2:
+            raise ValueError("l2g: contiguous int64 host tensor [nelem][Nm]")
+        if sign is not None and (sign.dtype != torch.int8 or sign.is_cuda or not sign.is_contiguous() or sign.shape != l2g.shape):
+            raise ValueError("sign: contiguous int8 host tensor of the shape of l2g")
+        h = _p()
+        _check(lib.nk_gs_create(l2g.shape[0], l2g.shape[1], int(nglobal), l2g.data_ptr(), sign.data_ptr() if sign is not None else None,
+                                C.byref(h)))
+        self.h, self.nelem, self.nm, self.nglobal = h, l2g.shape[0], l2g.shape[1], int(nglobal)
+
+    def close(self):
+        if self.h:
+            lib.nk_gs_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def gs_gather(gs, glob, local, stream=None):
+    _check(lib.nk_gs_gather(gs.h, _field(glob, gs.nglobal, "global"), _field(local, gs.nelem * gs.nm, "local"), _stream(stream)))
+
+
+def gs_scatter_add(gs, local, glob, stream=None):
+    _check(lib.nk_gs_scatter_add(gs.h, _field(local, gs.nelem * gs.nm, "local"), _field(glob, gs.nglobal, "global"), _stream(stream)))
+
+
+def assembled_helmholtz_apply(basis, geom, gs, lam, inp, out, stream=None):
+    _check(lib.nk_assembled_helmholtz_apply(basis.h, geom.h, gs.h, float(lam), _field(inp, gs.nglobal, "in"),
+                                            _field(out, gs.nglobal, "out"), _stream(stream)))
+
+
+PRECOND_NONE, PRECOND_JACOBI = 0, 1
+
+
+def cg_solve(basis, geom, gs, lam, rhs, x, rtol=1e-10, maxit=1000, precond=PRECOND_JACOBI, stream=None):
+    """returns (iterations, relative residual); x holds the initial guess on entry and the solution on return."""
+    it, rel = _i(), _d()
+    _check(lib.nk_cg_solve(basis.h, geom.h, gs.h, float(lam), _field(rhs, gs.nglobal, "rhs"), _field(x, gs.nglobal, "x"),
+                           int(precond), float(rtol), int(maxit), C.byref(it), C.byref(rel), _stream(stream)))
+    return it.value, rel.value
 
 
 def set_affine_simplex_form(form):

@@ -66,6 +66,8 @@ def build(force=False, jobs=None, verbose=False, extra_defs=(), lib=None, objdir
     dense_o = os.path.join(OBJ, "nk_dense.o")
     tasks.append((dense_o, [nvcc, *COMMON, *ARCH, *(["-Xptxas", "-v"] if verbose else []), "-c",
                             os.path.join(CSRC, "nk_dense.cu"), "-o", dense_o]))
+    sol_o = os.path.join(OBJ, "nk_solver.o")
+    tasks.append((sol_o, [nvcc, *COMMON, *ARCH, "-c", os.path.join(CSRC, "nk_solver.cu"), "-o", sol_o]))
     tab_o = os.path.join(OBJ, "nk_host_tables.o")
     tasks.append((tab_o, [nvcc, *COMMON, "-c", os.path.join(CSRC, "nk_host_tables.cpp"), "-o", tab_o]))
     for shape, pmax in MAX_P.items():

@@ -915,4 +915,11 @@ extern "C" int64_t nk_launch_count(void)
     return g_launches;
 }
 extern "C" const char* nk_last_error(void) { return g_err.c_str(); }
-extern "C" const char* nk_version(void) { return "libnk 0.1 (sm_100a)"; }
+// for the other translation units of the library (nk_solver.cu): not declared in nk.h
+extern "C" void nk_set_error_(const char* msg) { g_err = msg ? msg : ""; }
+extern "C" void nk_count_launches_(int n)
+{
+    std::lock_guard<std::mutex> lk(g_mutex);
+    g_launches += n;
+}
+extern "C" const char* nk_version(void) { return "libnk 0.2 (sm_100a)"; }

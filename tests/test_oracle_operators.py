@@ -378,3 +378,50 @@ def test_oracle_rounding_against_extended_precision(cfg):
         assert yld.dtype == np.longdouble
         err = (np.abs(y64 - yld).max(axis=1) / np.abs(yld).max(axis=1)).max()
         assert float(err) <= 1e-13, "%s: fp64 vs extended %.2e" % (title, float(err))
+
+
+def test_assembled_matrix_pins():
+    """oracle.assembled_matrix: one element reproduces L + lambda M; on a 2^3 mesh of deformed
+    hexes the matrix is symmetric positive definite, 1^T A 1 = lambda * volume (vertex modes of the connected
+    mesh sum to 1 and L 1 = 0), and a global trilinear function has the energy of its exact integrals."""
+    from workloads import assembly as asm
+    from workloads import synthetic as wl
+    P, lam, n = 2, 2.5, 2
+    el = o.Element(o.HEX, P, P + 2)
+    v0, E = wl.hex_mesh(n)
+    A, J = wl.affine_factors(v0, E)
+    A, J = A.numpy(), J.numpy()
+    l2g, ng = asm.hex_l2g(n, P)
+    l2g = l2g.numpy()
+    # one element on its own: the map is a permutation-free identity when numbered locally
+    M0, L0 = o.element_matrices(el, A[0], J[0])
+    A1 = o.assembled_matrix(el, A[:1], J[:1], lam, np.arange(el.Nm)[None, :], el.Nm)
+    assert np.abs(A1 - (L0 + lam * M0)).max() <= 1e-15 * np.abs(A1).max()
+    G = o.assembled_matrix(el, A, J, lam, l2g, ng)
+    assert np.abs(G - G.T).max() <= 1e-14 * np.abs(G).max()
+    assert np.linalg.eigvalsh(G).min() > 0
+    # the constant 1 on the connected mesh: coefficient 1 on every VERTEX dof, 0 elsewhere
+    one = np.zeros(ng)
+    N1 = n * P + 1
+    vid = [(gx * N1 + gy) * N1 + gz for gx in range(0, N1, P) for gy in range(0, N1, P) for gz in range(0, N1, P)]
+    one[vid] = 1.0
+    assert abs(one @ G @ one - lam * 1.0) <= 1e-13           # 1^T (L + lam M) 1 = lam * volume of the unit cube
+    assert np.abs(G @ one - lam * o.assembled_matrix(el, A, J, 1.0, l2g, ng) @ one + lam * o.assembled_matrix(el, A, J, 0.0, l2g, ng) @ one).max() <= 1e-13
+    assert np.abs(o.assembled_matrix(el, A, J, 0.0, l2g, ng) @ one).max() <= 1e-13     # L 1 = 0 on the assembled mesh
+    # u = x y z (trilinear, in the span of the vertex modes): energy = int |grad u|^2 + lam u^2 over the unit cube
+    h = 1.0 / n
+    u = np.zeros(ng)
+    for gx in range(0, N1, P):
+        for gy in range(0, N1, P):
+            for gz in range(0, N1, P):
+                u[(gx * N1 + gy) * N1 + gz] = (gx // P * h) * (gy // P * h) * (gz // P * h)
+    exact = 3.0 * (1.0 / 9.0) + lam * (1.0 / 27.0)            # int (yz)^2 + (xz)^2 + (xy)^2 = 3/9 ; int (xyz)^2 = 1/27
+    assert abs(u @ G @ u - exact) <= 1e-13
+    # signs: flipping the sign of one shared dof in every element that holds it flips the matching rows and columns
+    sign = np.ones_like(l2g, dtype=np.int8)
+    g0 = int(l2g[0, el.Nm - 1])
+    sign[l2g == g0] = -1
+    Gs = o.assembled_matrix(el, A, J, lam, l2g, ng, sign)
+    D = np.ones(ng)
+    D[g0] = -1.0
+    assert np.abs(Gs - D[:, None] * G * D[None, :]).max() <= 1e-15 * np.abs(G).max()
