@@ -138,11 +138,16 @@ nk_status dense_fragments(const nk_basis* b, int kind, const double** out)
 bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
 {
     *st = NK_OK;
-    if (deformed || b->t.shape == nk::HEX) return false;
+    if (deformed) return false;
     if (op != nk::OP_MASS && op != nk::OP_LAP && op != nk::OP_HELM && op != nk::OP_HELMF) return false;
     const int form = simplex_form();
     if (form == 1) return false;
-    const bool have = nk::dense_supported(b->t.Nm) && (b->t.shape == nk::TET || form == 2);
+    // automatic choice: every tet order, and the trilinear hex (P = 1: 7 x 64 FMA per element as 14 DMMA per 8 elements beat the
+    // Kronecker form's 272 FMA in 64-thread blocks with three barriers: config 4 P1, profiles/r2_notes.md); hexes of higher order
+    // keep the Kronecker forms (nm^4 against nm^6 work); other shapes only when form 2 asks for it
+    const bool autosel = b->t.shape == nk::TET || (b->t.shape == nk::HEX && b->t.P == 1);
+    if (b->t.shape == nk::HEX && b->t.P > 1) return false;
+    const bool have = nk::dense_supported(b->t.Nm) && (autosel || form == 2);
     if (!have && form == 2) *st = fail(NK_ERR_UNSUPPORTED, "no reference-matrix kernel for this (shape, P)");
     return have;
 }
@@ -738,8 +743,14 @@ extern "C" nk_status nk_helmholtz_apply_host(const nk_basis* b, const nk_geom* g
     // chunk unit: groups of the kernel (not of the stream), or tiles of 8 elements of the reference-matrix kernel
     const int Eop = dense ? 8 : g->deformed ? b->inst->E[1] : b->inst->E_op_affine[nk::OP_HELM];
     const int64_t ngroups_op = (g->nelem + Eop - 1) / Eop;
-    // at least ~2 MB per chunk: below that the per-copy latency costs more than the overlap gains
-    int nchunks = (int)std::min<int64_t>(nk_geom::kChunks, std::max<int64_t>(1, (int64_t)(bytes >> 21)));
+    // chunk size: NK_HOST_CHUNK_MB (default 8 MB; B200 sweep in profiles/r2_notes.md): smaller chunks pay the per-copy
+    // latency more often than the extra overlap gains
+    static const long long chunk_mb = [] {
+        const char* ev = std::getenv("NK_HOST_CHUNK_MB");
+        const long long v = ev ? std::atoll(ev) : 8;
+        return v < 1 ? 1LL : v;
+    }();
+    int nchunks = (int)std::min<int64_t>(nk_geom::kChunks, std::max<int64_t>(1, (int64_t)(bytes / ((size_t)chunk_mb << 20))));
     const int64_t per = (ngroups_op + nchunks - 1) / nchunks;
     const size_t elem_bytes = (size_t)Nm * sizeof(double);
     nk_status st = NK_OK;
