@@ -339,17 +339,26 @@ def measure_cg(nk, dev, barrier):
     return out
 
 
-def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budget_ms=400.0):
+def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budget_ms=100.0, gpu_index=0):
     """One entry of roofline.per_workload: the workload timed with the protocol of the headline (CUDA events, >= 3
-    warm-ups, rotating buffers), about `budget_ms` of kernel time."""
+    warm-ups, rotating buffers), about `budget_ms` of kernel time -- the length of the headline's own timed region
+    (400 x 0.08 ms): on this 1 kW part a loop of half a second runs into `sw_power_cap` (SM clock 1965 -> 1792 MHz,
+    config 5: 20.4 -> 19.3 GDoF/s), and the roofline denominators are burst figures.  SM clock and throttle reasons
+    are sampled during each entry's timed region."""
     import torch
     if name == "cg":
         return measure_cg(nk, dev, barrier)
+    time.sleep(0.2)     # let the power limiter recover from the previous entry
     w = Workload(nk, name, dev, rank)
     ms0 = timed(w.step, 3, 3, barrier)
-    steps = int(max(10, min(2000, budget_ms / max(ms0, 1e-4))))
+    steps = int(max(20, min(2000, budget_ms / max(ms0, 1e-4))))
+    sampler = ClockSampler(gpu_index)
+    sampler.start()
     ms = timed(w.step, steps, 5, barrier)
+    sampler.stop_flag = True
+    sampler.join()
     out = {"workload": w.title, "op": w.op, "steps": steps, "ms": ms, "value": w.dof / (ms * 1e-3) / 1e9, "unit": "GDoF/s",
+           "clocks": sampler.result(),
            "algorithmic_bytes": w.alg["bytes"], "algorithmic_flops": w.alg["flops"], "running_form_flops": w.alg["flops_run"]}
     out.update(fractions(w.alg, ms, hbm_peak, fp64_tf))
     if w.op == "mass+laplacian":          # config 4: each operator on its own, both flop counts (SURVEY 8(d) and the running form)
@@ -572,7 +581,7 @@ def main():
         pw = {}
         for name in names:
             try:
-                pw[name] = measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf)
+                pw[name] = measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, gpu_index=physical_gpu_index(local))
             except Exception as ex:
                 pw[name] = {"error": str(ex)[:200]}
         roof["per_workload"] = pw

@@ -90,12 +90,29 @@ struct Tune {
     static constexpr int RING = (DEF && SHAPE != K_HEX && Q >= 10) ? 2 : 0;
 #endif
     static constexpr size_t smem_ring = (size_t)NT * RING * 7 * sizeof(double);
+    // EARLY: number of k-planes of the thread's pass-C line whose 7 metric entries are requested BEFORE the barrier in
+    // front of pass C (registers held across it), so that their L2 latency overlaps the wait at the barrier
+    // (nk_stage_mid.inc; B200 sweep in profiles/r2_notes.md section 7)
+#if defined(NK_TUNE_EARLY)
+    static constexpr int EARLY = (DEF && RING == 0) ? (NK_TUNE_EARLY < Q ? NK_TUNE_EARLY : Q) : 0;
+#else
+    static constexpr int EARLY = (DEF && RING == 0) ? (SHAPE != K_HEX ? 1 : Q == 9 ? 2 : 0) : 0;
+#endif
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
-    static constexpr int REGS = DEF ? (SHAPE == K_HEX ? 96 : 72) : Q <= 6 ? 56 : 64;
-    static constexpr int MINB_smem = (int)((220 * 1024) / (smem_grid + smem_ring + 2048));
+    // registers per thread asked of ptxas (through the blocks-per-SM bound); round-2 sweep of the bound on every
+    // deformed workload (profiles/r2_notes.md section 7): hexes 96 except Q = 4 (64: cfg2:2 +4 %), Q = 7 and Q = 10
+    // (80: cfg2:5 +5 %, cfg2:8 +7 %); simplices 72 except Q = 6 and Q = 8 (64: cfg5:4 +6 %, cfg5:6 +12 %, where 64
+    // registers let a second 512-thread block fit)
+#if defined(NK_TUNE_REGS)
+    static constexpr int REGS = NK_TUNE_REGS;
+#else
+    static constexpr int REGS = DEF ? (SHAPE == K_HEX ? (Q == 4 ? 64 : (Q == 7 || Q == 10) ? 80 : 96) : (Q == 6 || Q == 8) ? 64 : 72)
+                                    : Q <= 6 ? 56 : 64;
+#endif
+    static constexpr int MINB_smem = (int)((227 * 1024) / (smem_grid + smem_ring + 1024));
     static constexpr int MINB_reg = 65536 / (NT * REGS);
     static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
 #endif
