@@ -339,12 +339,13 @@ def measure_cg(nk, dev, barrier):
     return out
 
 
-def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budget_ms=100.0, gpu_index=0):
+def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budget_ms=40.0, gpu_index=0):
     """One entry of roofline.per_workload: the workload timed with the protocol of the headline (CUDA events, >= 3
     warm-ups, rotating buffers), about `budget_ms` of kernel time -- the length of the headline's own timed region
-    (400 x 0.08 ms): on this 1 kW part a loop of half a second runs into `sw_power_cap` (SM clock 1965 -> 1792 MHz,
-    config 5: 20.4 -> 19.3 GDoF/s), and the roofline denominators are burst figures.  SM clock and throttle reasons
-    are sampled during each entry's timed region."""
+    (400 x 0.08 ms = 33 ms): on this 1 kW part longer loops run into the power limiter (config 5: 20.8 GDoF/s over 40
+    steps, 20.4 over 100, 19.3 over 400 with `sw_power_cap` and the SM clock at 1792 MHz), and the roofline
+    denominators are burst figures.  Entries are separated by short pauses; SM clock and throttle reasons are sampled
+    during each entry's timed region."""
     import torch
     if name == "cg":
         return measure_cg(nk, dev, barrier)
@@ -365,6 +366,7 @@ def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budge
         basis, geom, xs, ys, _, ne = w.work[0]
         b0 = w.blocks[0]
         for opname, fn in (("mass", nk.mass_apply), ("laplacian", nk.laplacian_apply)):
+            time.sleep(0.3)
             ms1 = timed(lambda i: fn(basis, geom, xs[i % NSETS], ys[i % NSETS]), steps, 3, barrier)
             a = algorithmic(b0["shape"], b0["P"], b0["deformed"], opname)
             a = {k: v * ne for k, v in a.items()}
@@ -374,9 +376,14 @@ def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budge
     elif len(w.work) > 1:                  # config 5: each block's launch on its own
         out["blocks"] = []
         for (basis, geom, xs, ys, l, ne), blk in zip(w.work, w.per_block):
-            ms1 = timed(lambda i: nk.helmholtz_apply(basis, geom, l, xs[i % NSETS], ys[i % NSETS]), steps, 3, barrier)
+            time.sleep(0.3)
+            smp = ClockSampler(gpu_index)
+            smp.start()
+            ms1 = timed(lambda i: nk.helmholtz_apply(basis, geom, l, xs[i % NSETS], ys[i % NSETS]), max(20, steps // 2), 3, barrier)
+            smp.stop_flag = True
+            smp.join()
             r = {"shape": ("hex", "tet", "prism")[blk["shape"]], "P": blk["P"], "nelem": ne, "ms": ms1,
-                 "value": blk["dof"] / (ms1 * 1e-3) / 1e9}
+                 "value": blk["dof"] / (ms1 * 1e-3) / 1e9, "clocks": smp.result()}
             r.update(fractions(blk, ms1, hbm_peak, fp64_tf))
             out["blocks"].append(r)
     if w.dof < 100000:                     # config 1 (64 elements): latency per call, eager and as a CUDA graph of 20 calls
