@@ -202,7 +202,9 @@ nk_status nk_cg_solve(const nk_basis* b, const nk_geom* g, const nk_gs* gs, doub
  * nk_helmholtz_* call on an AFFINE simplex block take
  *   form 0 (default)  the reference-matrix kernel where one is instantiated (tets), else the sum-factorised kernel,
  *   form 1            the sum-factorised kernel (Eq. 17 / 21 / 23 step by step, as on deformed blocks),
- *   form 2            the reference-matrix kernel; NK_ERR_UNSUPPORTED at apply time where none is instantiated.
+ *   form 2            the reference-matrix kernel on EVERY affine block (prisms and hexes of any order too): where no kernel
+ *                     is prebuilt for the block's number of modes, the kernel source is specialised for it at run time
+ *                     (NVRTC, next paragraph); NK_ERR_UNSUPPORTED at apply time if that is not possible.
  * Process-wide; the initial value is the environment variable NK_SIMPLEX_FORM (0 if unset).                     */
 nk_status nk_set_affine_simplex_form(int form);
 int nk_get_affine_simplex_form(void);
@@ -210,6 +212,16 @@ int nk_get_affine_simplex_form(void);
  * c = 0 (1,1), 1 (1,2)+(2,1), 2 (1,3)+(3,1), 3 (2,2), 4 (2,3)+(3,2), 5 (3,3): sum_q w_q d_a phi_m d_b phi_n in
  * standard-element coordinates; c = 6: sum_q w_q phi_m phi_n.  Built on first use (host only; needs no GPU).   */
 nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, double* host_out, size_t cap);
+
+/* ---- run-time specialisation (the paper's JIT: "< 1 second" P:350) ----------------
+ * The reference-matrix kernels depend on one number, the modes per element.  For a mode count outside the prebuilt
+ * table (tets P1..P8, trilinear hexes) libnk compiles csrc/nk_dense.cuh with NVRTC for exactly that count on first use,
+ * loads the cubin through the driver API and caches it per (device, modes, operator).  libnvrtc and libcuda are
+ * dlopen'ed: no link-time dependency.  The sum-factorised kernels are NOT specialised at run time (Q = P+2 table only).
+ * nk_jit_compile_check: compile the Helmholtz kernel for `nmodes` without loading it (needs NO GPU): NVRTC's wall time in
+ * ms and the cubin size.  nk_jit_stats: kernels specialised for launching so far in this process and their compile time. */
+nk_status nk_jit_compile_check(int nmodes, double* compile_ms, size_t* cubin_bytes);
+nk_status nk_jit_stats(int64_t* kernels, double* compile_ms);
 
 /* ---- diagnostics ----------------------------------------------------------------------------- */
 /* Register-only DFMA chains on every SM for `iters` x 1024 FMAs per thread (8 independent chains); *tflops receives the

@@ -49,6 +49,8 @@ _SIG = {
     "nk_gs_scatter_add": (_i, [_p, _p, _p, _p]),
     "nk_assembled_helmholtz_apply": (_i, [_p, _p, _p, _d, _p, _p, _p]),
     "nk_cg_solve": (_i, [_p, _p, _p, _d, _p, _p, _i, _d, _i, C.POINTER(_i), C.POINTER(_d), _p]),
+    "nk_jit_compile_check": (_i, [_i, C.POINTER(_d), C.POINTER(_sz)]),
+    "nk_jit_stats": (_i, [C.POINTER(_i64), C.POINTER(_d)]),
     "nk_set_affine_simplex_form": (_i, [_i]),
     "nk_get_affine_simplex_form": (_i, []),
     "nk_basis_get_reference_matrix": (_i, [_p, _i, C.POINTER(_d), _sz]),
@@ -330,6 +332,20 @@ def cg_solve(basis, geom, gs, lam, rhs, x, rtol=1e-10, maxit=1000, precond=PRECO
     _check(lib.nk_cg_solve(basis.h, geom.h, gs.h, float(lam), _field(rhs, gs.nglobal, "rhs"), _field(x, gs.nglobal, "x"),
                            int(precond), float(rtol), int(maxit), C.byref(it), C.byref(rel), _stream(stream)))
     return it.value, rel.value
+
+
+def jit_compile_check(nmodes):
+    """(compile ms, cubin bytes) of the NVRTC specialisation of the reference-matrix Helmholtz kernel; needs no GPU."""
+    ms, nb = _d(), _sz()
+    _check(lib.nk_jit_compile_check(int(nmodes), C.byref(ms), C.byref(nb)))
+    return ms.value, nb.value
+
+
+def jit_stats():
+    """(kernels specialised at run time for launching so far, their total NVRTC time in ms)"""
+    k, ms = _i64(), _d()
+    _check(lib.nk_jit_stats(C.byref(k), C.byref(ms)))
+    return k.value, ms.value
 
 
 def set_affine_simplex_form(form):

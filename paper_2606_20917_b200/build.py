@@ -66,6 +66,14 @@ def build(force=False, jobs=None, verbose=False, extra_defs=(), lib=None, objdir
     dense_o = os.path.join(OBJ, "nk_dense.o")
     tasks.append((dense_o, [nvcc, *COMMON, *ARCH, *(["-Xptxas", "-v"] if verbose else []), "-c",
                             os.path.join(CSRC, "nk_dense.cu"), "-o", dense_o]))
+    # the text of nk_dense.cuh as a C++ raw string literal, for the NVRTC path of nk_jit.cu
+    src_inc = os.path.join(OBJ, "nk_dense_src.inc")
+    text = 'R"NKSRC(' + open(os.path.join(CSRC, "nk_dense.cuh")).read() + ')NKSRC"\n'
+    if not os.path.exists(src_inc) or open(src_inc).read() != text:
+        with open(src_inc, "w") as f:
+            f.write(text)
+    jit_o = os.path.join(OBJ, "nk_jit.o")
+    tasks.append((jit_o, [nvcc, *COMMON, *ARCH, "-I", OBJ, "-c", os.path.join(CSRC, "nk_jit.cu"), "-o", jit_o]))
     sol_o = os.path.join(OBJ, "nk_solver.o")
     tasks.append((sol_o, [nvcc, *COMMON, *ARCH, "-c", os.path.join(CSRC, "nk_solver.cu"), "-o", sol_o]))
     tab_o = os.path.join(OBJ, "nk_host_tables.o")
@@ -87,7 +95,7 @@ def build(force=False, jobs=None, verbose=False, extra_defs=(), lib=None, objdir
                 logs.append(out)
     objs = [t[0] for t in tasks]
     if todo or _stale(LIB, objs):
-        _run([nvcc, "-shared", *ARCH, "-o", LIB, *objs, "-lcudart"])
+        _run([nvcc, "-shared", *ARCH, "-o", LIB, *objs, "-lcudart", "-ldl"])
     return "\n".join(logs)
 
 

@@ -133,8 +133,8 @@ nk_status dense_fragments(const nk_basis* b, int kind, const double** out)
     *out = b->d_frag[kind];
     return NK_OK;
 }
-// does this (basis, geometry, operator) take the reference-matrix kernel?  *st receives an error if form 2 is forced
-// where no kernel exists.
+// does this (basis, geometry, operator) take the reference-matrix kernel?  Form 2 on a mode count outside the
+// prebuilt table is served by a run-time specialisation (NVRTC, csrc/nk_jit.cu); its errors surface at launch.
 bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
 {
     *st = NK_OK;
@@ -146,10 +146,9 @@ bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
     // Kronecker form's 272 FMA in 64-thread blocks with three barriers: config 4 P1, profiles/r2_notes.md); hexes of higher order
     // keep the Kronecker forms (nm^4 against nm^6 work); other shapes only when form 2 asks for it
     const bool autosel = b->t.shape == nk::TET || (b->t.shape == nk::HEX && b->t.P == 1);
-    if (b->t.shape == nk::HEX && b->t.P > 1) return false;
-    const bool have = nk::dense_supported(b->t.Nm) && (autosel || form == 2);
-    if (!have && form == 2) *st = fail(NK_ERR_UNSUPPORTED, "no reference-matrix kernel for this (shape, P)");
-    return have;
+    if (b->t.shape == nk::HEX && b->t.P > 1 && form != 2) return false;
+    if (form == 2) return true;                              // prebuilt, or specialised at run time
+    return nk::dense_supported(b->t.Nm) && autosel;
 }
 } // namespace
 
@@ -541,8 +540,16 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
         if (d.e0 < 0 || d.e0 > nelem) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": bad tile range");
         d.scale6 = (kind == nk::DENSE_MASS) ? 1.0 : lambda;
         int launched = 0;
-        cudaError_t e = nk::dense_launch(b->t.Nm, kind, d, (cudaStream_t)stream, &launched);
-        if (e != cudaSuccess) return cuda_fail(e, name);
+        if (nk::dense_supported(b->t.Nm)) {
+            cudaError_t e = nk::dense_launch(b->t.Nm, kind, d, (cudaStream_t)stream, &launched);
+            if (e != cudaSuccess) return cuda_fail(e, name);
+        } else {
+            // mode count outside the prebuilt table: NVRTC specialisation of the same kernel source, cached
+            std::string why;
+            if (!nk::dense_jit_launch(b->t.Nm, kind, d, (cudaStream_t)stream, &launched, &why))
+                return fail(NK_ERR_UNSUPPORTED, std::string(name) + ": no reference-matrix kernel for this (shape, P) and run-time "
+                                                                    "specialisation failed: " + why);
+        }
         if (launched) { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
         return NK_OK;
     }
@@ -814,6 +821,23 @@ extern "C" nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, dou
     if (cap < n) return fail(NK_ERR_INVALID_ARG, "nk_basis_get_reference_matrix: capacity too small");
     const std::vector<double>& K7 = reference_matrices(b);
     std::memcpy(host_out, K7.data() + (size_t)c * n, n * sizeof(double));
+    return NK_OK;
+}
+
+extern "C" nk_status nk_jit_compile_check(int nmodes, double* compile_ms, size_t* cubin_bytes)
+{
+    if (nmodes < 1 || nmodes > 1024) return fail(NK_ERR_INVALID_ARG, "nk_jit_compile_check: 1 <= nmodes <= 1024");
+    std::string why;
+    if (!nk::dense_jit_compile_check(nmodes, nk::DENSE_HELM, compile_ms, cubin_bytes, &why)) return fail(NK_ERR_UNSUPPORTED, why);
+    return NK_OK;
+}
+extern "C" nk_status nk_jit_stats(int64_t* kernels, double* compile_ms)
+{
+    long long k = 0;
+    double ms = 0.0;
+    nk::dense_jit_stats(&k, &ms);
+    if (kernels) *kernels = k;
+    if (compile_ms) *compile_ms = ms;
     return NK_OK;
 }
 

@@ -21,8 +21,12 @@
 // tile per remaining mode m' whose 8 columns are the MATRICES c (B[k][c] = K_c[m'][4 ks + k], unscaled A), and the
 // sum over c with the weights G_c^e is taken across the four lanes of a quad by two warp shuffles.
 #pragma once
+// This header is also compiled at RUN TIME by NVRTC (csrc/nk_jit.cu: mode counts outside the prebuilt table); NVRTC
+// predefines the CUDA built-ins and has no host headers, so everything host-side is fenced with __CUDACC_RTC__.
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
 #include <stdint.h>
+#endif
 
 namespace nk {
 
@@ -224,7 +228,7 @@ struct DenseStream {
     static constexpr int STAGE_DOUBLES = MAIN_CHUNK_DOUBLES > REM_CHUNK_DOUBLES ? MAIN_CHUNK_DOUBLES : REM_CHUNK_DOUBLES;
     static constexpr int USTRIDE = (4 * S::NK) % 8 == 4 ? 4 * S::NK : 4 * S::NK + 4;   // = 4 mod 8: conflict-free A reads
     static constexpr int SLAB_DOUBLES = 8 * USTRIDE + 64;               // u[8][USTRIDE] + g[8][8]
-    static constexpr size_t smem_bytes(int warps, int stages)
+    __host__ __device__ static constexpr size_t smem_bytes(int warps, int stages)
     {
         return ((size_t)stages * STAGE_DOUBLES + (size_t)warps * SLAB_DOUBLES) * sizeof(double) + 2 * stages * sizeof(unsigned long long);
     }
@@ -409,6 +413,7 @@ __global__ void __launch_bounds__((WARPS + 1) * 32, MINB) nk_dense_stream_kernel
     }
 }
 
+#ifndef __CUDACC_RTC__
 // host: pack the symmetric matrices Kc[c][m][n] (c = 0..6, row-major Nm x Nm each) into fragment order for
 // DenseShape<NMODES, C0, NC>.  out must hold TOTAL_DOUBLES.
 inline void dense_pack(const double* K7, int nmodes, int c0, int nc, double* out)
@@ -438,5 +443,6 @@ inline size_t dense_pack_size(int nmodes, int nc)
     const int NTS = NTF + ((R > 0 && !REM) ? 1 : 0), NRT = REM ? R : 0;
     return (size_t)nc * NK * NTS * 32 + (size_t)NK * NRT * 32;
 }
+#endif // !__CUDACC_RTC__
 
 } // namespace nk

@@ -18,4 +18,15 @@ bool dense_supported(int nmodes);
 // *launched is set to 1 if a kernel was enqueued (0 for an empty range).
 cudaError_t dense_launch(int nmodes, int kind, const DenseArgs& a, cudaStream_t stream, int* launched);
 
+// ---- run-time specialisation (csrc/nk_jit.cu): NVRTC compiles nk_dense.cuh for a mode count outside the table ----
+} // namespace nk
+#include <string>
+namespace nk {
+// compiles (cached per device, Nm, kind) and launches; false + *err on any failure (no NVRTC, no driver, compile error)
+bool dense_jit_launch(int nmodes, int kind, const DenseArgs& a, cudaStream_t stream, int* launched, std::string* err);
+// compiles only (needs no GPU): time in ms and size of the cubin
+bool dense_jit_compile_check(int nmodes, int kind, double* ms, size_t* cubin_bytes, std::string* err);
+// kernels compiled for launching so far in this process, and the time NVRTC took for them
+void dense_jit_stats(long long* kernels, double* total_ms);
+
 } // namespace nk

@@ -160,3 +160,19 @@ def test_simplex_form_option():
             nk.set_affine_simplex_form(3)
     finally:
         nk.set_affine_simplex_form(old)
+
+
+@pytest.mark.parametrize("nmodes", [6, 27, 75, 126])
+def test_runtime_specialisation_compiles_without_a_gpu(nmodes):
+    """nk_jit_compile_check: NVRTC compiles the reference-matrix kernel for a mode count outside
+    the prebuilt table (prism P1, hex P2, prism P4 -> streamed variant, prism P5), on a machine without a GPU, in less
+    than the paper's budget for its JIT ("< 1 second"; a generous 5 s here for a loaded CI host)."""
+    try:
+        ms, nbytes = nk.jit_compile_check(nmodes)
+    except nk.NkError as e:
+        if "libnvrtc not found" in str(e):
+            pytest.skip("libnvrtc is not installed here")
+        raise
+    assert nbytes > 10000 and 0 < ms < 5000.0
+    with pytest.raises(nk.NkError):
+        nk.jit_compile_check(0)
