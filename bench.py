@@ -84,7 +84,7 @@ def algorithmic(shape, P, deformed, op="helmholtz", form=0):
             run = 6 * nm ** 4 + Nm
         elif P <= 7:                     # 17 nm x nm contractions per line set (nk_stage_lapkron.inc)
             run = 2 * 17 * nm ** 4 + 12 * Nm
-    if not deformed and form != 1 and (shape == 1 or (shape == 0 and P == 1)):
+    if not deformed and form != 1 and (shape == 1 or (shape == 0 and P == 1) or (shape == 2 and P <= 3)):
         nc = 1 if op == "mass" else 6 if op == "laplacian" else 7    # reference-matrix GEMM (nk_dense.cuh): tets, trilinear hexes
         run = 2 * nc * Nm * Nm
     return {"bytes": by, "flops": fl, "flops_run": run}

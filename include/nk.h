@@ -200,7 +200,8 @@ nk_status nk_cg_solve(const nk_basis* b, const nk_geom* g, const nk_gs* gs, doub
  * a dense GEMM with a fixed right-hand matrix, run on the FP64 tensor cores (DMMA) for tets up to P = 5 where it
  * needs fewer flops than the sum-factorised chain.  nk_mass_apply, nk_laplacian_apply and every
  * nk_helmholtz_* call on an AFFINE simplex block take
- *   form 0 (default)  the reference-matrix kernel where one is instantiated (tets), else the sum-factorised kernel,
+ *   form 0 (default)  the reference-matrix kernel where it is the faster one (tets of every order, prisms up to P = 3,
+ *                     trilinear hexes), else the sum-factorised / Kronecker kernel,
  *   form 1            the sum-factorised kernel (Eq. 17 / 21 / 23 step by step, as on deformed blocks),
  *   form 2            the reference-matrix kernel on EVERY affine block (prisms and hexes of any order too): where no kernel
  *                     is prebuilt for the block's number of modes, the kernel source is specialised for it at run time

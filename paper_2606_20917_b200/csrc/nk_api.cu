@@ -145,7 +145,8 @@ bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
     // automatic choice: every tet order, and the trilinear hex (P = 1: 7 x 64 FMA per element as 14 DMMA per 8 elements beat the
     // Kronecker form's 272 FMA in 64-thread blocks with three barriers: config 4 P1, profiles/r2_notes.md); hexes of higher order
     // keep the Kronecker forms (nm^4 against nm^6 work); other shapes only when form 2 asks for it
-    const bool autosel = b->t.shape == nk::TET || (b->t.shape == nk::HEX && b->t.P == 1);
+    // prisms up to P = 3 (Nm = 6, 18, 40: 92 / 84 / 54 against 34 / 43 / 41 GDoF/s for the chain; at P = 4, Nm = 75, the chain wins)
+    const bool autosel = b->t.shape == nk::TET || (b->t.shape == nk::HEX && b->t.P == 1) || (b->t.shape == nk::PRISM && b->t.P <= 3);
     if (b->t.shape == nk::HEX && b->t.P > 1 && form != 2) return false;
     if (form == 2) return true;                              // prebuilt, or specialised at run time
     return nk::dense_supported(b->t.Nm) && autosel;

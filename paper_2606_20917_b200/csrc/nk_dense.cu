@@ -110,6 +110,7 @@ struct DenseInst {
 // Nm = 84, 120, 165: tets P6..P8; matrices streamed from L2 (consumer warps, k-steps per chunk, ring stages, blocks/SM).
 const DenseInst kInst[] = {
     NK_DENSE_ROW(8, 8, 4),         // hex P1 (the 8 vertex modes): 14 DMMA per 8 elements, HBM-bound
+    NK_DENSE_ROW(6, 8, 4),         NK_DENSE_ROW(18, 8, 4),          NK_DENSE_ROW(40, 16, 1),         // prisms P1..P3
     NK_DENSE_ROW(4, 8, 4),         NK_DENSE_ROW(10, 16, 2),         NK_DENSE_ROW(20, 8, 3),          NK_DENSE_ROW(35, 16, 1),
     NK_DENSE_ROW(56, 16, 1),       NK_STREAM_ROW(84, 4, 7, 2, 3),   NK_STREAM_ROW(120, 8, 5, 3, 1),  NK_STREAM_ROW(165, 4, 6, 2, 2),
 };
