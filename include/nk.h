@@ -171,6 +171,12 @@ typedef struct nk_gs nk_gs;
 nk_status nk_gs_create(int64_t nelem, int nm_local, int64_t nglobal, const int64_t* l2g, const signed char* sign, nk_gs** out);
 nk_status nk_gs_destroy(nk_gs* gs);
 int64_t nk_gs_num_global(const nk_gs* gs);
+/* Constrained (Dirichlet) dofs: HOST list of n global dofs (n = 0 removes the constraints).  nk_assembled_helmholtz_apply
+ * and nk_cg_solve then work with A_c = P A P + (I - P), P = projector on the free dofs: identity rows and columns at the
+ * constrained dofs, so A_c is symmetric positive definite also for lambda = 0 (Poisson) once the boundary is held, and
+ * the solution equals the right-hand side at the constrained dofs (0 for homogeneous conditions; for inhomogeneous ones
+ * the caller moves A_fc x_c to the right-hand side).  nk_gs_gather / nk_gs_scatter_add themselves ignore the constraints. */
+nk_status nk_gs_set_constrained(nk_gs* gs, int64_t n, const int64_t* dofs);
 /* local = Q global: device [nglobal] -> device [nelem][nm_local]                                                  */
 nk_status nk_gs_gather(const nk_gs* gs, const double* global, double* local, void* stream);
 /* global = Q^T local (overwrites global).  Deterministic: one thread per global dof sums its local copies in the
@@ -179,7 +185,8 @@ nk_status nk_gs_scatter_add(const nk_gs* gs, const double* local, double* global
 /* out = Q^T (L + lambda M) Q in on device vectors [nglobal]: gather, ONE fused elemental kernel, scatter.          */
 nk_status nk_assembled_helmholtz_apply(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* in,
                                        double* out, void* stream);
-/* Conjugate gradients on A x = rhs, A as above (symmetric positive definite for lambda > 0; no constrained dofs).
+/* Conjugate gradients on A x = rhs, A as above or its constrained form A_c (symmetric positive definite for lambda > 0,
+ * or for lambda = 0 with enough constrained dofs).
  * precond: NK_PRECOND_NONE, or NK_PRECOND_JACOBI = diag(A)^-1 with diag(A) = Q^T diag(H^e); the elemental diagonals are
  * obtained by applying the elemental operator to the Nm unit vectors (Nm launches, once per (geometry, lambda), cached in
  * the nk_gs handle).  The modified basis is badly conditioned without it (16^3 deformed hexes at P4, lambda = 1, to

@@ -420,3 +420,14 @@ def assembled_matrix(el, dxi_dx, detJ, lam, l2g, nglobal, sign=None):
             for n in range(el.Nm):
                 A[l2g[e, m], l2g[e, n]] += H[m, n]
     return A
+
+
+def constrained_matrix(A, dofs):
+    """A_c = P A P + (I - P), P = projector on the dofs NOT in `dofs`: rows and columns of the constrained dofs replaced
+    by those of the identity (homogeneous Dirichlet conditions).  Pins: equals A on the free-free block, identity on the
+    constrained block, zero between them; the Poisson matrix (lambda = 0) with the whole boundary held is positive definite."""
+    Ac = A.copy()
+    Ac[dofs, :] = 0.0
+    Ac[:, dofs] = 0.0
+    Ac[dofs, dofs] = 1.0
+    return Ac

@@ -45,6 +45,7 @@ _SIG = {
     "nk_gs_create": (_i, [_i64, _i, _i64, _p, _p, C.POINTER(_p)]),
     "nk_gs_destroy": (_i, [_p]),
     "nk_gs_num_global": (_i64, [_p]),
+    "nk_gs_set_constrained": (_i, [_p, _i64, _p]),
     "nk_gs_gather": (_i, [_p, _p, _p, _p]),
     "nk_gs_scatter_add": (_i, [_p, _p, _p, _p]),
     "nk_assembled_helmholtz_apply": (_i, [_p, _p, _p, _d, _p, _p, _p]),
@@ -297,6 +298,12 @@ class GatherScatter:
         _check(lib.nk_gs_create(l2g.shape[0], l2g.shape[1], int(nglobal), l2g.data_ptr(), sign.data_ptr() if sign is not None else None,
                                 C.byref(h)))
         self.h, self.nelem, self.nm, self.nglobal = h, l2g.shape[0], l2g.shape[1], int(nglobal)
+
+    def set_constrained(self, dofs):
+        """dofs: int64 CPU tensor of constrained (Dirichlet) global dofs; empty removes the constraints."""
+        if dofs.dtype != torch.int64 or dofs.is_cuda or not dofs.is_contiguous():
+            raise ValueError("dofs: contiguous int64 host tensor")
+        _check(lib.nk_gs_set_constrained(self.h, dofs.numel(), dofs.data_ptr() if dofs.numel() else None))
 
     def close(self):
         if self.h:

@@ -21,20 +21,28 @@ namespace {
 
 enum { kRedBlocks = 592, kRedThreads = 256 };   // 4 blocks per SM of a B200; the grid is FIXED so that sums are reproducible
 
-__global__ void gather_kernel(const int* __restrict__ l2g, const signed char* __restrict__ sgn, const double* __restrict__ glob,
-                              double* __restrict__ loc, long long n)
+// free: optional [nglobal] flags, 1 = free dof, 0 = constrained (reads as 0: the operator acts on the free dofs only)
+__global__ void gather_kernel(const int* __restrict__ l2g, const signed char* __restrict__ sgn, const unsigned char* __restrict__ free,
+                              const double* __restrict__ glob, double* __restrict__ loc, long long n)
 {
     for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) {
-        const double v = __ldg(glob + l2g[i]);
+        const int g = l2g[i];
+        const double v = (!free || free[g]) ? __ldg(glob + g) : 0.0;
         loc[i] = sgn ? (sgn[i] < 0 ? -v : v) : v;
     }
 }
 
 // global[g] = sum over the local copies of g, in the order of the transposed map (CSR: rowptr, col = local index)
+// free / ident: a constrained dof takes ident[g] (identity row of the constrained operator) or 1 if ident is NULL
 __global__ void scatter_kernel(const long long* __restrict__ rowptr, const int* __restrict__ col, const signed char* __restrict__ sgn,
-                               const double* __restrict__ loc, double* __restrict__ glob, long long nglobal)
+                               const double* __restrict__ loc, double* __restrict__ glob, long long nglobal,
+                               const unsigned char* __restrict__ free = nullptr, const double* __restrict__ ident = nullptr)
 {
     for (long long g = blockIdx.x * (long long)blockDim.x + threadIdx.x; g < nglobal; g += (long long)gridDim.x * blockDim.x) {
+        if (free && !free[g]) {
+            glob[g] = ident ? ident[g] : 1.0;
+            continue;
+        }
         double s = 0.0;
         for (long long k = rowptr[g]; k < rowptr[g + 1]; ++k) {
             const int c = col[k];
@@ -160,6 +168,7 @@ struct nk_gs {
     signed char* d_sgn = nullptr;    // [nlocal] or NULL (all +1)
     long long* d_rowptr = nullptr;   // [nglobal + 1]
     int* d_col = nullptr;            // [nlocal]
+    unsigned char* d_free = nullptr; // [nglobal] 1 = free, 0 = constrained; NULL = no constraints (nk_gs_set_constrained)
     // work space of nk_assembled_apply / nk_cg_solve (allocated on first use, under mu)
     std::mutex mu;
     double *d_lin = nullptr, *d_lout = nullptr, *d_r = nullptr, *d_p = nullptr, *d_Ap = nullptr, *d_partial = nullptr, *d_sc = nullptr;
@@ -219,7 +228,7 @@ extern "C" nk_status nk_gs_create(int64_t nelem, int nm_local, int64_t nglobal, 
 extern "C" nk_status nk_gs_destroy(nk_gs* gs)
 {
     if (!gs) return NK_OK;
-    for (void* p : {(void*)gs->d_l2g, (void*)gs->d_sgn, (void*)gs->d_rowptr, (void*)gs->d_col, (void*)gs->d_lin, (void*)gs->d_lout,
+    for (void* p : {(void*)gs->d_free, (void*)gs->d_l2g, (void*)gs->d_sgn, (void*)gs->d_rowptr, (void*)gs->d_col, (void*)gs->d_lin, (void*)gs->d_lout,
                     (void*)gs->d_r, (void*)gs->d_p, (void*)gs->d_Ap, (void*)gs->d_partial, (void*)gs->d_sc, (void*)gs->d_z, (void*)gs->d_diag,
                     (void*)gs->d_ldiag})
         if (p) cudaFree(p);
@@ -228,6 +237,28 @@ extern "C" nk_status nk_gs_destroy(nk_gs* gs)
 }
 
 extern "C" int64_t nk_gs_num_global(const nk_gs* gs) { return gs ? gs->nglobal : -1; }
+
+extern "C" nk_status nk_gs_set_constrained(nk_gs* gs, int64_t n, const int64_t* dofs)
+{
+    if (!gs || n < 0 || (n > 0 && !dofs)) return sfail(NK_ERR_INVALID_ARG, "nk_gs_set_constrained: bad arguments");
+    std::lock_guard<std::mutex> lk(gs->mu);
+    gs->diag_geom = nullptr;                       // the cached Jacobi diagonal belongs to the old constraint set
+    if (n == 0) {
+        if (gs->d_free) cudaFree(gs->d_free);
+        gs->d_free = nullptr;
+        return NK_OK;
+    }
+    std::vector<unsigned char> f((size_t)gs->nglobal, 1);
+    for (int64_t i = 0; i < n; ++i) {
+        if (dofs[i] < 0 || dofs[i] >= gs->nglobal) return sfail(NK_ERR_INVALID_ARG, "nk_gs_set_constrained: dof out of range");
+        f[(size_t)dofs[i]] = 0;
+    }
+    cudaError_t e = cudaSuccess;
+    if (!gs->d_free) e = cudaMalloc(&gs->d_free, (size_t)gs->nglobal);
+    if (e == cudaSuccess) e = cudaMemcpy(gs->d_free, f.data(), (size_t)gs->nglobal, cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) return sfail(NK_ERR_CUDA, std::string("nk_gs_set_constrained: ") + cudaGetErrorString(e));
+    return NK_OK;
+}
 
 static int grid_for(long long n)
 {
@@ -239,7 +270,7 @@ extern "C" nk_status nk_gs_gather(const nk_gs* gs, const double* global, double*
 {
     if (!gs || (gs->nlocal > 0 && (!global || !local))) return sfail(NK_ERR_INVALID_ARG, "nk_gs_gather: NULL argument");
     if (gs->nlocal == 0) return NK_OK;
-    gather_kernel<<<grid_for(gs->nlocal), 256, 0, (cudaStream_t)stream>>>(gs->d_l2g, gs->d_sgn, global, local, gs->nlocal);
+    gather_kernel<<<grid_for(gs->nlocal), 256, 0, (cudaStream_t)stream>>>(gs->d_l2g, gs->d_sgn, nullptr, global, local, gs->nlocal);
     nk_count_launches_(1);
     const cudaError_t e = cudaGetLastError();
     return e == cudaSuccess ? NK_OK : sfail(NK_ERR_CUDA, std::string("nk_gs_gather: ") + cudaGetErrorString(e));
@@ -275,13 +306,18 @@ static nk_status ensure_work(nk_gs* gs)
     return NK_OK;
 }
 
-// out = Q^T H Q in on the caller's stream; work space of gs (callers hold gs->mu)
+// out = A in on the caller's stream, A = Q^T H Q, or with constrained dofs A = P Q^T H Q P + (I - P) (P = projector on
+// the free dofs: identity rows and columns at the constrained ones); work space of gs (callers hold gs->mu)
 static nk_status assembled_apply(const nk_basis* b, const nk_geom* g, nk_gs* gs, double lambda, const double* in, double* out, void* stream)
 {
-    nk_status st = nk_gs_gather(gs, in, gs->d_lin, stream);
-    if (st == NK_OK) st = nk_helmholtz_apply(b, g, lambda, gs->d_lin, gs->d_lout, stream);
-    if (st == NK_OK) st = nk_gs_scatter_add(gs, gs->d_lout, out, stream);
-    return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    gather_kernel<<<grid_for(gs->nlocal), 256, 0, s>>>(gs->d_l2g, gs->d_sgn, gs->d_free, in, gs->d_lin, gs->nlocal);
+    nk_status st = nk_helmholtz_apply(b, g, lambda, gs->d_lin, gs->d_lout, stream);
+    if (st != NK_OK) return st;
+    scatter_kernel<<<grid_for(gs->nglobal), 256, 0, s>>>(gs->d_rowptr, gs->d_col, gs->d_sgn, gs->d_lout, out, gs->nglobal, gs->d_free, in);
+    nk_count_launches_(2);
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? NK_OK : sfail(NK_ERR_CUDA, std::string("assembled apply: ") + cudaGetErrorString(e));
 }
 
 extern "C" nk_status nk_assembled_helmholtz_apply(const nk_basis* b, const nk_geom* g, const nk_gs* gsc, double lambda, const double* in,
@@ -314,7 +350,7 @@ static nk_status assembled_diagonal(const nk_basis* b, const nk_geom* g, nk_gs* 
         nk_count_launches_(2);
     }
     // signs square to one: the plain transposed sum (a map without signs)
-    scatter_kernel<<<grid_for(gs->nglobal), 256, 0, s>>>(gs->d_rowptr, gs->d_col, nullptr, gs->d_ldiag, gs->d_diag, gs->nglobal);
+    scatter_kernel<<<grid_for(gs->nglobal), 256, 0, s>>>(gs->d_rowptr, gs->d_col, nullptr, gs->d_ldiag, gs->d_diag, gs->nglobal, gs->d_free, nullptr);
     nk_count_launches_(1);
     const cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return sfail(NK_ERR_CUDA, std::string("nk_cg_solve: diagonal: ") + cudaGetErrorString(e));

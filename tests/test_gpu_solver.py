@@ -90,6 +90,39 @@ def test_assembled_apply_and_cg_against_dense_oracle(nk, P, deformed, precond):
     assert it3 == 0
 
 
+@pytest.mark.parametrize("P", [2, 4])
+def test_poisson_with_dirichlet_boundary(nk, P):
+    """lambda = 0 with the boundary dofs constrained (nk_gs_set_constrained): the assembled apply and the CG solve against
+    the oracle's constrained matrix; removing the constraints restores the plain operator."""
+    n = 2
+    el, A, J, basis, geom, l2g, ng = setup(nk, n, P, True)
+    bd = asm.hex_boundary_dofs(n, P)
+    L = o.assembled_matrix(el, A.numpy(), J.numpy(), 0.0, l2g.numpy(), ng)
+    Lc = o.constrained_matrix(L, bd.numpy())
+    gs = nk.GatherScatter(l2g, ng)
+    gs.set_constrained(bd)
+    rng = np.random.Generator(np.random.Philox(31 + P))
+    u = rng.standard_normal(ng)
+    out = torch.full((ng,), float("nan"), dtype=torch.float64, device="cuda")
+    nk.assembled_helmholtz_apply(basis, geom, gs, 0.0, torch.from_numpy(u).cuda(), out)
+    ref = Lc @ u
+    assert np.abs(out.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+    b = rng.standard_normal(ng)
+    b[bd.numpy()] = 0.0                                             # homogeneous conditions
+    for precond in (0, 1):
+        x = torch.zeros(ng, dtype=torch.float64, device="cuda")
+        iters, rel = nk.cg_solve(basis, geom, gs, 0.0, torch.from_numpy(b).cuda(), x, rtol=1e-10, maxit=20 * ng, precond=precond)
+        xs = np.linalg.solve(Lc, b)
+        assert rel <= 1e-10 and float(x[bd.cuda()].abs().max()) == 0.0
+        assert np.abs(x.cpu().numpy() - xs).max() <= 10 * np.linalg.cond(Lc) * 1e-10 * np.abs(xs).max()
+    gs.set_constrained(torch.zeros(0, dtype=torch.int64))
+    nk.assembled_helmholtz_apply(basis, geom, gs, 0.0, torch.from_numpy(u).cuda(), out)
+    ref = L @ u
+    assert np.abs(out.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+    with pytest.raises(nk.NkError):
+        gs.set_constrained(torch.tensor([ng], dtype=torch.int64))
+
+
 def test_cg_larger_mesh_residual(nk):
     """a mesh the dense oracle cannot hold (16^3 deformed hexes, P4, 2.7e5 dofs): CG converges and the residual,
     recomputed through the parity-tested assembled apply, matches the one the solver reports."""

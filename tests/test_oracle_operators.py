@@ -425,3 +425,24 @@ def test_assembled_matrix_pins():
     D = np.ones(ng)
     D[g0] = -1.0
     assert np.abs(Gs - D[:, None] * G * D[None, :]).max() <= 1e-15 * np.abs(G).max()
+
+
+def test_constrained_matrix_pins():
+    from workloads import assembly as asm
+    from workloads import synthetic as wl
+    P, n = 2, 2
+    el = o.Element(o.HEX, P, P + 2)
+    v0, E = wl.hex_mesh(n)
+    A, J = wl.affine_factors(v0, E)
+    l2g, ng = asm.hex_l2g(n, P)
+    bd = asm.hex_boundary_dofs(n, P).numpy()
+    N1 = n * P + 1
+    assert len(bd) == N1 ** 3 - (N1 - 2) ** 3 and len(set(bd.tolist())) == len(bd)
+    L = o.assembled_matrix(el, A.numpy(), J.numpy(), 0.0, l2g.numpy(), ng)
+    assert np.linalg.eigvalsh(L).min() < 1e-12                     # pure Neumann Laplacian: singular (constants)
+    Lc = o.constrained_matrix(L, bd)
+    free = np.setdiff1d(np.arange(ng), bd)
+    assert np.array_equal(Lc[np.ix_(free, free)], L[np.ix_(free, free)])
+    assert np.array_equal(Lc[np.ix_(bd, bd)], np.eye(len(bd)))
+    assert not Lc[np.ix_(bd, free)].any() and not Lc[np.ix_(free, bd)].any()
+    assert np.linalg.eigvalsh(Lc).min() > 1e-6                     # boundary held: positive definite (8e-5 here)

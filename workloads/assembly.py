@@ -23,3 +23,13 @@ def hex_l2g(n, P):
     l2g = (gx * N1 + gy) * N1 + gz
     l2g = l2g.expand(n, n, n, nm, nm, nm).reshape(n ** 3, nm ** 3).contiguous().to(torch.int64)
     return l2g, N1 ** 3
+
+
+def hex_boundary_dofs(n, P):
+    """global dofs of hex_l2g(n, P) that lie on the boundary of the unit cube (a 1-D index 0 or n*P in any direction):
+    int64 tensor, ascending"""
+    N1 = n * P + 1
+    g = torch.arange(N1)
+    on = (g == 0) | (g == N1 - 1)
+    m = on[:, None, None] | on[None, :, None] | on[None, None, :]
+    return torch.nonzero(m.reshape(-1)).reshape(-1).to(torch.int64).contiguous()
