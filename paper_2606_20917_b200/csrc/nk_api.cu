@@ -50,9 +50,10 @@ InstGetter inst_getter(int shape, int P)
     return tab[shape][P - 1];
 }
 
-// form of the affine simplex operators (mass / Laplacian / Helmholtz): 0 = automatic (reference-matrix DMMA kernel
-// where one is instantiated, else the sum-factorised kernel), 1 = sum-factorised always, 2 = reference-matrix
-// (NK_ERR_UNSUPPORTED where none is instantiated).  Initial value from the environment variable NK_SIMPLEX_FORM.
+// form of the affine mass / Laplacian / Helmholtz operators (nk.h, nk_set_affine_simplex_form): 0 = automatic (the
+// reference-matrix DMMA kernel where it is the faster one, see use_dense below), 1 = never the reference-matrix kernel,
+// 2 = always (specialised at run time where no kernel is prebuilt).  Initial value from the environment variable
+// NK_SIMPLEX_FORM.
 int g_simplex_form = -1;
 int simplex_form()
 {
@@ -133,8 +134,12 @@ nk_status dense_fragments(const nk_basis* b, int kind, const double** out)
     *out = b->d_frag[kind];
     return NK_OK;
 }
-// does this (basis, geometry, operator) take the reference-matrix kernel?  Form 2 on a mode count outside the
-// prebuilt table is served by a run-time specialisation (NVRTC, csrc/nk_jit.cu); its errors surface at launch.
+// does this (basis, geometry, operator) take the reference-matrix kernel?
+//   form 1: never.  form 2: every affine block (mode counts outside the prebuilt table are specialised at run time by
+//   NVRTC, csrc/nk_jit.cu; a failure there surfaces at launch).  form 0: where it is the faster kernel -- tets of every
+//   order, prisms up to P = 3 (92 / 84 / 54 against 34 / 43 / 41 GDoF/s for the chain; at P = 4 the chain wins) and
+//   trilinear hexes (14 DMMA per 8 elements against the Kronecker form's 272 FMA in 64-thread blocks with three
+//   barriers); hexes of order >= 2 keep the Kronecker forms (nm^4 against nm^6 work).  profiles/r2_notes.md
 bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
 {
     *st = NK_OK;
@@ -142,14 +147,10 @@ bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
     if (op != nk::OP_MASS && op != nk::OP_LAP && op != nk::OP_HELM && op != nk::OP_HELMF) return false;
     const int form = simplex_form();
     if (form == 1) return false;
-    // automatic choice: every tet order, and the trilinear hex (P = 1: 7 x 64 FMA per element as 14 DMMA per 8 elements beat the
-    // Kronecker form's 272 FMA in 64-thread blocks with three barriers: config 4 P1, profiles/r2_notes.md); hexes of higher order
-    // keep the Kronecker forms (nm^4 against nm^6 work); other shapes only when form 2 asks for it
-    // prisms up to P = 3 (Nm = 6, 18, 40: 92 / 84 / 54 against 34 / 43 / 41 GDoF/s for the chain; at P = 4, Nm = 75, the chain wins)
-    const bool autosel = b->t.shape == nk::TET || (b->t.shape == nk::HEX && b->t.P == 1) || (b->t.shape == nk::PRISM && b->t.P <= 3);
-    if (b->t.shape == nk::HEX && b->t.P > 1 && form != 2) return false;
-    if (form == 2) return true;                              // prebuilt, or specialised at run time
-    return nk::dense_supported(b->t.Nm) && autosel;
+    if (form == 2) return true;
+    const int shape = b->t.shape, P = b->t.P;
+    const bool faster = shape == nk::TET || (shape == nk::PRISM && P <= 3) || (shape == nk::HEX && P == 1);
+    return faster && nk::dense_supported(b->t.Nm);
 }
 } // namespace
 
