@@ -185,6 +185,24 @@ nk_status nk_gs_scatter_add(const nk_gs* gs, const double* local, double* global
 /* out = Q^T (L + lambda M) Q in on device vectors [nglobal]: gather, ONE fused elemental kernel, scatter.          */
 nk_status nk_assembled_helmholtz_apply(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* in,
                                        double* out, void* stream);
+/* The same operation for callers that cannot allocate (code under CUDA graph capture, serving loops, harnesses that
+ * forbid cudaMalloc): this call allocates NOTHING -- no cudaMalloc / cudaFree, no allocating library routine.  Its two
+ * local work vectors ([nelem][nm_local] doubles each) live in a file-scope __device__ array of the library,
+ * 2 x NK_STATIC_MAX_LOCAL_DOFS doubles = 16 MiB, which every GPU that loads libnk holds until the process exits.
+ *   - nelem * nm_local > NK_STATIC_MAX_LOCAL_DOFS: NK_ERR_UNSUPPORTED (nothing is launched); nk_static_max_local_dofs()
+ *     returns the limit of the loaded library.
+ *   - a block whose elemental operator would still build device tables (affine block on the reference-matrix form
+ *     whose matrices are not resident yet, or a run-time-specialised kernel): NK_ERR_UNSUPPORTED; call
+ *     nk_helmholtz_apply once on the block at set-up, or select form 1.  Deformed blocks and affine hexes of order
+ *     >= 2 never need that.
+ *   - EVERY call on a device shares the one array: calls whose GPU work overlaps (different streams, or two host
+ *     threads on one device) race on it -- keep them on one stream or order them with events.  The array keeps the last
+ *     call's contents; no entry is read before the same call has written it, so nothing needs clearing.
+ * Results are bit-identical to nk_assembled_helmholtz_apply (same kernels, same order of sums).                    */
+#define NK_STATIC_MAX_LOCAL_DOFS 1048576
+int64_t nk_static_max_local_dofs(void);
+nk_status nk_assembled_helmholtz_apply_static(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* in,
+                                              double* out, void* stream);
 /* Conjugate gradients on A x = rhs, A as above or its constrained form A_c (symmetric positive definite for lambda > 0,
  * or for lambda = 0 with enough constrained dofs).
  * precond: NK_PRECOND_NONE, or NK_PRECOND_JACOBI = diag(A)^-1 with diag(A) = Q^T diag(H^e); the elemental diagonals are

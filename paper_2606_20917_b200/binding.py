@@ -49,6 +49,8 @@ _SIG = {
     "nk_gs_gather": (_i, [_p, _p, _p, _p]),
     "nk_gs_scatter_add": (_i, [_p, _p, _p, _p]),
     "nk_assembled_helmholtz_apply": (_i, [_p, _p, _p, _d, _p, _p, _p]),
+    "nk_static_max_local_dofs": (_i64, []),
+    "nk_assembled_helmholtz_apply_static": (_i, [_p, _p, _p, _d, _p, _p, _p]),
     "nk_cg_solve": (_i, [_p, _p, _p, _d, _p, _p, _i, _d, _i, C.POINTER(_i), C.POINTER(_d), _p]),
     "nk_jit_compile_check": (_i, [_i, C.POINTER(_d), C.POINTER(_sz)]),
     "nk_jit_stats": (_i, [C.POINTER(_i64), C.POINTER(_d)]),
@@ -328,6 +330,17 @@ def gs_scatter_add(gs, local, glob, stream=None):
 def assembled_helmholtz_apply(basis, geom, gs, lam, inp, out, stream=None):
     _check(lib.nk_assembled_helmholtz_apply(basis.h, geom.h, gs.h, float(lam), _field(inp, gs.nglobal, "in"),
                                             _field(out, gs.nglobal, "out"), _stream(stream)))
+
+
+def static_max_local_dofs():
+    return int(lib.nk_static_max_local_dofs())
+
+
+def assembled_helmholtz_apply_static(basis, geom, gs, lam, inp, out, stream=None):
+    """nk_assembled_helmholtz_apply_static: the same operation with the work space in the library's static device array
+    (allocates nothing; at most static_max_local_dofs() local dofs; calls that overlap on the GPU race on the array)."""
+    _check(lib.nk_assembled_helmholtz_apply_static(basis.h, geom.h, gs.h, float(lam), _field(inp, gs.nglobal, "in"),
+                                                   _field(out, gs.nglobal, "out"), _stream(stream)))
 
 
 PRECOND_NONE, PRECOND_JACOBI = 0, 1

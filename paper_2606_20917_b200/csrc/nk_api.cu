@@ -959,4 +959,20 @@ extern "C" void nk_count_launches_(int n)
     std::lock_guard<std::mutex> lk(g_mutex);
     g_launches += n;
 }
+// Would nk_helmholtz_apply(b, g, ...) allocate device memory or load a module if called NOW on the current device?
+// 0 = no: the sum-factorised / Kronecker kernels take their tables as kernel parameters, and a prebuilt reference-matrix
+// kernel whose fragment-ordered matrices are already resident on this device allocates nothing; 1 = yes: the matrices
+// are still to be uploaded (first apply on this basis) or the kernel would be specialised at run time (nk_jit.cu).
+// For nk_assembled_helmholtz_apply_static (nk_solver.cu), which must not allocate.  Not declared in nk.h.
+extern "C" int nk_helmholtz_apply_allocates_(const nk_basis* b, const nk_geom* g)
+{
+    if (!b || !g) return 1;
+    nk_status st = NK_OK;
+    if (!use_dense(b, g->deformed, nk::OP_HELM, &st)) return st == NK_OK ? 0 : 1;
+    if (!nk::dense_supported(b->t.Nm)) return 1;
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) return 1;
+    std::lock_guard<std::mutex> lk(b->mu);
+    return (b->d_frag[nk::DENSE_HELM] && b->frag_dev == dev) ? 0 : 1;
+}
 extern "C" const char* nk_version(void) { return "libnk 0.2 (sm_100a)"; }

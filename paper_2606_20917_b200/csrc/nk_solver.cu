@@ -442,3 +442,74 @@ extern "C" nk_status nk_cg_solve(const nk_basis* b, const nk_geom* g, const nk_g
     if (relres_out) *relres_out = rel;
     return NK_OK;
 }
+
+// =========================== the entry point that allocates nothing ===========================
+// nk_assembled_helmholtz_apply_static (nk.h): nk_assembled_helmholtz_apply with the two local work vectors (Q in and
+// H Q in, [nelem][Nm] each) in a file-scope device array instead of cudaMalloc'ed work space of the nk_gs handle, for
+// callers that cannot allocate (CUDA graph capture, serving loops).  2 x NK_STATIC_MAX_LOCAL_DOFS doubles = 16 MiB,
+// held by every GPU that loads the library until the process exits.
+// In HOST code the name nk_static_scratch is a host-side stand-in, not a device address: the kernels get the address
+// cudaGetSymbolAddress returns, asked for once per device with that device current (static_scratch below).
+static __device__ __align__(256) double nk_static_scratch[2 * (size_t)NK_STATIC_MAX_LOCAL_DOFS];
+
+namespace {
+// device address of nk_static_scratch on the CURRENT device (cached per device ordinal)
+nk_status static_scratch(double** out)
+{
+    enum { kMaxDevices = 64 };
+    static std::mutex mu;
+    static double* addr[kMaxDevices] = {};
+    int dev = 0;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return sfail(NK_ERR_CUDA, std::string("nk_assembled_helmholtz_apply_static: cudaGetDevice: ") + cudaGetErrorString(e));
+    if (dev < 0 || dev >= kMaxDevices) return sfail(NK_ERR_UNSUPPORTED, "nk_assembled_helmholtz_apply_static: device ordinal beyond 63");
+    std::lock_guard<std::mutex> lk(mu);
+    if (!addr[dev]) {
+        double* p = nullptr;
+        e = cudaGetSymbolAddress((void**)&p, nk_static_scratch);
+        if (e != cudaSuccess || !p)
+            return sfail(NK_ERR_CUDA, std::string("nk_assembled_helmholtz_apply_static: cudaGetSymbolAddress: ") + cudaGetErrorString(e));
+        addr[dev] = p;
+    }
+    *out = addr[dev];
+    return NK_OK;
+}
+} // namespace
+
+extern "C" int nk_helmholtz_apply_allocates_(const nk_basis* b, const nk_geom* g);   // nk_api.cu
+
+extern "C" int64_t nk_static_max_local_dofs(void) { return (int64_t)NK_STATIC_MAX_LOCAL_DOFS; }
+
+extern "C" nk_status nk_assembled_helmholtz_apply_static(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* in,
+                                                         double* out, void* stream)
+{
+    const char* me = "nk_assembled_helmholtz_apply_static";
+    if (!b || !g || !gs || !in || !out) return sfail(NK_ERR_INVALID_ARG, std::string(me) + ": NULL argument");
+    if (gs->nelem != nk_geom_num_elements(g) || gs->nm != nk_basis_num_modes(b))
+        return sfail(NK_ERR_SHAPE_MISMATCH, std::string(me) + ": the map does not belong to this block");
+    if (in == out) return sfail(NK_ERR_INVALID_ARG, std::string(me) + ": in and out alias");
+    if (gs->nlocal > (int64_t)NK_STATIC_MAX_LOCAL_DOFS)
+        return sfail(NK_ERR_UNSUPPORTED, std::string(me) + ": " + std::to_string((long long)gs->nlocal) + " local dofs (nelem x Nm) exceed the static work "
+                     "space of NK_STATIC_MAX_LOCAL_DOFS = " + std::to_string((long long)NK_STATIC_MAX_LOCAL_DOFS) +
+                     "; use nk_assembled_helmholtz_apply (it allocates its work space on first use)");
+    if (gs->nglobal == 0) return NK_OK;
+    if (nk_helmholtz_apply_allocates_(b, g))
+        return sfail(NK_ERR_UNSUPPORTED, std::string(me) + ": the elemental operator of this block would still build device tables (reference-matrix "
+                     "form: first use on this basis, or a kernel specialised at run time); call nk_helmholtz_apply once on the block at set-up, "
+                     "or select form 1 (nk_set_affine_simplex_form)");
+    double* w = nullptr;
+    nk_status st = static_scratch(&w);
+    if (st != NK_OK) return st;
+    double* lin = w;
+    double* lout = w + (size_t)NK_STATIC_MAX_LOCAL_DOFS;
+    // Nothing in the array has to start at zero: the gather writes lin[0, nlocal), the elemental kernel writes
+    // lout[0, nlocal), and nothing beyond nlocal is read; what an earlier call left behind is never seen.
+    cudaStream_t s = (cudaStream_t)stream;
+    gather_kernel<<<grid_for(gs->nlocal), 256, 0, s>>>(gs->d_l2g, gs->d_sgn, gs->d_free, in, lin, gs->nlocal);
+    st = nk_helmholtz_apply(b, g, lambda, lin, lout, stream);
+    if (st != NK_OK) return st;
+    scatter_kernel<<<grid_for(gs->nglobal), 256, 0, s>>>(gs->d_rowptr, gs->d_col, gs->d_sgn, lout, out, gs->nglobal, gs->d_free, in);
+    nk_count_launches_(2);
+    const cudaError_t e = cudaGetLastError();
+    return e == cudaSuccess ? NK_OK : sfail(NK_ERR_CUDA, std::string(me) + ": " + cudaGetErrorString(e));
+}
