@@ -178,11 +178,10 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
                 NK_FOR(l, NM * NM) {
                     double c[NM];
                     NK_UNROLL for (int r = 0; r < NM; ++r) c[r] = Y[(l * NM + r) * E + e];
-                    NK_UNROLL for (int k = 0; k < Q; ++k) {
-                        double acc = 0.0;
-                        NK_UNROLL for (int r = 0; r < NM; ++r) acc = fma(tabs.Ba[2][k * NM + r], c[r], acc);
-                        Z[T1IDX(l, k)] = acc;
-                    }
+                    double t1[Q];
+                    zero(t1);
+                    contract<T::COLS, Q, NM>(tabs.Ba[2], tabs.BaT[2], c, t1);
+                    NK_UNROLL for (int k = 0; k < Q; ++k) Z[T1IDX(l, k)] = t1[k];
                 }
             } else {
 #define NK_SX_STAGE 1
@@ -196,11 +195,10 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
                     const int p = l / Q, k = l - p * Q;
                     double c[NM];
                     NK_UNROLL for (int q = 0; q < NM; ++q) c[q] = Z[T1IDX(p * NM + q, k)];
-                    NK_UNROLL for (int j = 0; j < Q; ++j) {
-                        double acc = 0.0;
-                        NK_UNROLL for (int q = 0; q < NM; ++q) acc = fma(tabs.Ba[1][j * NM + q], c[q], acc);
-                        X[T2IDX(p, j, k)] = acc;
-                    }
+                    double t2[Q];
+                    zero(t2);
+                    contract<T::COLS, Q, NM>(tabs.Ba[1], tabs.BaT[1], c, t2);
+                    NK_UNROLL for (int j = 0; j < Q; ++j) X[T2IDX(p, j, k)] = t2[j];
                 }
             } else {
 #define NK_SX_STAGE 2

@@ -98,6 +98,15 @@ struct Tune {
 #else
     static constexpr int EARLY = (DEF && RING == 0) ? (SHAPE != K_HEX ? 1 : Q == 9 ? 2 : 0) : 0;
 #endif
+    // COLS: form of the 1-D contractions (contract below): input-outermost over the transposed tables
+#if defined(NK_TUNE_COLS)
+    static constexpr bool COLS = NK_TUNE_COLS != 0;
+#else
+    // B200 sweep over every order (profiles/r2_notes.md section 10): wins where ptxas' uniform-register shuffle is heavy --
+    // hexes from Q = 10 (deformed P8 / P9 / P10 +5 / +11 / +14 %; affine Laplacian P8 / P10 +8 / +14 %, P9 -2 %) and
+    // simplices from Q = 9 (config 5 P7 / P8 +3 / +9 %); below, the two forms are within 1-3 % and the row form stays
+    static constexpr bool COLS = SHAPE == K_HEX ? (Q >= 10 && (DEF || Q != 11)) : Q >= 9;
+#endif
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
@@ -137,6 +146,13 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
     static constexpr bool LAP_KRON = AFF_HEX && (P + 1) <= NK_LAPKRON_MAXNM && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
 #endif
     static constexpr bool KRON = MASS_KRON || LAP_KRON;
+#if defined(NK_TUNE_KCOLS)
+    static constexpr bool KCOLS = NK_TUNE_KCOLS != 0;
+#else
+    // coefficient-space kernels (same sweep): mass from nm = 9 on (P8..P10 +4..6 %), Laplacian / Helmholtz up to nm = 6
+    // (P3 / P4 / P5 +6 / +2 / +15 %); at nm = 7, 8 the column form of stage 1 adds local-memory spills to stage 2's
+    static constexpr bool KCOLS = MASS_KRON ? (P + 1) >= 9 : (P + 1) <= 6;
+#endif
     static constexpr int NM = P + 1;
 #if defined(NK_TUNE_EMASS)
     static constexpr int EK = NK_TUNE_EMASS;
@@ -248,6 +264,35 @@ __device__ __forceinline__ void static_switch(int v, F&& f)
 }
 
 #define NK_UNROLL _Pragma("unroll")
+// acc[o] += sum_r M[o][r] * in[r]: a register line times a constant-bank 1-D matrix, given both as M ([o][r], row-major)
+// and as its transpose MT ([r][o], contiguous in the OUTPUT index).
+//   COLS = false: output-outermost over M (one dot product after the other in the source).
+//   COLS = true:  input-outermost over MT.
+// ptxas runs the NOUT accumulators side by side whatever the source order.  From the row-major table it then fetches
+// pairs along the INPUT index (LDCU.128), parks their second halves in uniform registers and shuffles them with UMOV:
+// 0.6 UMOV per DFMA at Q = 12 and uniform-register spills from Q = 9 on, a quarter of all instructions of the deformed
+// hex P10 kernel (profiles/r2_notes.md section 10).  With MT every LDCU.128 pair feeds the next two DFMA and dies.
+// The order of every single sum (r ascending) is the same in both forms: results are bit-identical.
+template <bool COLS, int NOUT, int NIN>
+__device__ __forceinline__ void contract(const double* __restrict__ M, const double* __restrict__ MT, const double (&in)[NIN],
+                                         double (&acc)[NOUT])
+{
+    if constexpr (COLS) {
+        NK_UNROLL for (int r = 0; r < NIN; ++r)
+            NK_UNROLL for (int o = 0; o < NOUT; ++o) acc[o] = fma(MT[r * NOUT + o], in[r], acc[o]);
+    } else {
+        NK_UNROLL for (int o = 0; o < NOUT; ++o) {
+            double a = acc[o];
+            NK_UNROLL for (int r = 0; r < NIN; ++r) a = fma(M[o * NIN + r], in[r], a);
+            acc[o] = a;
+        }
+    }
+}
+template <int N>
+__device__ __forceinline__ void zero(double (&v)[N])
+{
+    NK_UNROLL for (int i = 0; i < N; ++i) v[i] = 0.0;
+}
 // line loop of a stage: thread `slot` takes lines slot, slot+LS, ...  The trip count is a compile-time
 // constant so that single-trip stages are straight-line code.
 // NK_FORU: the same, fully unrolled (global loads/stores: all trips in flight at once)
