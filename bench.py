@@ -2,7 +2,7 @@
 """bench.py -- Helmholtz-apply throughput (GDoF/s, fp64) of libnk on B200, with the roofline fraction of
 the kernel and the CPU oracle timed beside it.  Contract: see DESIGN.md section 8.
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2[:P]|cfg3[:P]|cfg4:P|cfg5[:P]]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg1|cfg2[:P[:Q]]|cfg3[:P[:Q]]|cfg4:P[:Q]|cfg5[:P[:Q]]]
                     [--per-workload default|none] [--impl reference]
 
 A step = one pass of the whole hot path (ONE fused kernel per block) over the
@@ -45,10 +45,16 @@ def parse_args():
 
 def workload_blocks(name, device, rank=0):
     from workloads import configs as cfgs          # data generators only
-    P = int(name.split(":")[1]) if ":" in name else None       # cfg4:P (and cfg2:P, cfg3:P, cfg5:P): the P-sweep
+    parts = name.split(":")
+    P = int(parts[1]) if len(parts) > 1 else None       # cfg4:P (and cfg2:P, cfg3:P, cfg5:P): the P-sweep
     title, op, blocks = cfgs.config_blocks(int(name[3:4]), device=device, P_sweep=P)
     for b in blocks:
         b["seed"] += 1000 * rank
+        b["Q"] = b["P"] + 2
+    if len(parts) > 2:                                   # cfgN:P:Q -- the same mesh with Q points per direction (kernels
+        for b in blocks:                                 # outside the Q = P+2 table are specialised at run time)
+            b["Q"] = int(parts[2])
+            title = title.replace("Q%d" % (b["P"] + 2), "Q%d" % b["Q"])
     return title, op, blocks
 
 
@@ -57,11 +63,11 @@ def nmodes(shape, P):
     return nm ** 3 if shape == 0 else nm * (nm + 1) * (nm + 2) // 6 if shape == 1 else nm * nm * (nm + 1) // 2
 
 
-def algorithmic(shape, P, deformed, op="helmholtz", form=0):
+def algorithmic(shape, P, deformed, op="helmholtz", form=0, Q=None):
     """Per element: bytes the METHOD must move, the flops of SURVEY 8(d)'s sum-factorised chain (`flops`: the
     contract's algorithmic count) and the flops of the form that actually runs (`flops_run`; DESIGN.md section 5:
     the coefficient-space forms of the affine operators need fewer)."""
-    nm, Q = P + 1, P + 2
+    nm, Q = P + 1, (P + 2 if Q is None else Q)
     Nm, Nq = nmodes(shape, P), Q ** 3
     if shape == 0:
         bwd = 2 * (nm ** 3 * Q + nm ** 2 * Q ** 2 + nm * Q ** 3)
@@ -157,17 +163,17 @@ def oracle_leg(workload, budget_s, want_steps=None, warmup=0, chunk=256):
     cores = os.cpu_count() or 1
     per_block = []
     for b in blocks:
-        el = o.Element(b["shape"], b["P"], b["P"] + 2)
+        el = o.Element(b["shape"], b["P"], b["Q"])
         take = min(b["v0"].shape[0], chunk * cores)
         A, J = (wl.sinusoidal_factors(b["v0"][:take], b["E"][:take], el.xi) if b["deformed"]
                 else wl.affine_factors(b["v0"][:take], b["E"][:take]))
         x = wl.coefficients(b["seed"], take, el.Nm).numpy()
-        per_block.append((b["shape"], b["P"], A.numpy(), J.numpy(), x, b["lam"], take, el.Nm))
+        per_block.append((b["shape"], b["P"], b["Q"], A.numpy(), J.numpy(), x, b["lam"], take, el.Nm))
     with op_.OraclePool(cores) as pool:
         def one_pass():
             dof = 0
-            for shape, P, A, J, x, lam, take, Nm in per_block:
-                pool.apply("helmholtz", shape, P, P + 2, A, J, lam, x, chunk=max(1, -(-take // cores)), want_result=False)
+            for shape, P, Q, A, J, x, lam, take, Nm in per_block:
+                pool.apply("helmholtz", shape, P, Q, A, J, lam, x, chunk=max(1, -(-take // cores)), want_result=False)
                 dof += take * Nm
             return dof
 
@@ -228,7 +234,7 @@ class Workload:
         self.alg = {"bytes": 0, "flops": 0, "flops_run": 0}
         self.per_block = []
         for b in self.blocks:
-            basis = nk.Basis(b["shape"], b["P"])
+            basis = nk.Basis(b["shape"], b["P"], b["Q"])
             A, J = cfgs.block_factors(b, basis.points())
             geom = nk.Geom(basis, A, J, b["deformed"], streams=nk.Geom.METRIC)
             ne = J.shape[0]
@@ -239,7 +245,7 @@ class Workload:
             ops = ("mass", "laplacian") if self.op == "mass+laplacian" else ("helmholtz",)
             blk = {"bytes": 0, "flops": 0, "flops_run": 0}
             for o_ in ops:
-                a = algorithmic(b["shape"], b["P"], b["deformed"], o_, form)
+                a = algorithmic(b["shape"], b["P"], b["deformed"], o_, form, b["Q"])
                 blk["bytes"] += (a["bytes"] + 16 * basis.num_modes * (fields - 1)) * ne     # the geometry is shared by the fields
                 blk["flops"] += a["flops"] * ne * fields
                 blk["flops_run"] += a["flops_run"] * ne * fields
@@ -368,7 +374,7 @@ def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budge
         for opname, fn in (("mass", nk.mass_apply), ("laplacian", nk.laplacian_apply)):
             time.sleep(0.3)
             ms1 = timed(lambda i: fn(basis, geom, xs[i % NSETS], ys[i % NSETS]), steps, 3, barrier)
-            a = algorithmic(b0["shape"], b0["P"], b0["deformed"], opname)
+            a = algorithmic(b0["shape"], b0["P"], b0["deformed"], opname, 0, b0["Q"])
             a = {k: v * ne for k, v in a.items()}
             r = {"ms": ms1, "value": ne * basis.num_modes / (ms1 * 1e-3) / 1e9}
             r.update(fractions(a, ms1, hbm_peak, fp64_tf))

@@ -65,8 +65,10 @@ typedef struct nk_geom nk_geom;   /* opaque: nelem, deformed flag, repacked devi
 
 /* ---- basis / quadrature precompute (host only; needs no GPU) ----------------------------------
  * Modified C0 basis (A7, A8) with Gauss-Lobatto-Legendre points on hexes, GLL x Gauss-Radau-Jacobi(1,0)
- * x GRJ(2,0) on tets, GLL x GLL x GRJ(1,0) on prisms (A9).  Supported: Q == P+2 with
- * hex P in 1..10, tet and prism P in 1..8; anything else returns NK_ERR_UNSUPPORTED.               */
+ * x GRJ(2,0) on tets, GLL x GLL x GRJ(1,0) on prisms (A9).  Prebuilt kernels: Q == P+2 with
+ * hex P in 1..10, tet and prism P in 1..8.  Any other (P, Q) with 1 <= P <= 10, P+1 <= Q <= 12 whose tables fit the
+ * kernel-parameter space (every hex; tets / prisms up to P = 9) is accepted too and its kernels are specialised at
+ * run time on first use ("run-time specialisation" below); anything else returns NK_ERR_UNSUPPORTED.   */
 nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** out);
 nk_status nk_basis_destroy(nk_basis* b);
 int nk_basis_num_modes(const nk_basis* b);  /* Nm; -1 if b is NULL */
@@ -240,13 +242,21 @@ int nk_get_affine_simplex_form(void);
 nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, double* host_out, size_t cap);
 
 /* ---- run-time specialisation (the paper's JIT: "< 1 second" P:350) ----------------
- * The reference-matrix kernels depend on one number, the modes per element.  For a mode count outside the prebuilt
- * table (tets P1..P8, trilinear hexes) libnk compiles csrc/nk_dense.cuh with NVRTC for exactly that count on first use,
- * loads the cubin through the driver API and caches it per (device, modes, operator).  libnvrtc and libcuda are
- * dlopen'ed: no link-time dependency.  The sum-factorised kernels are NOT specialised at run time (Q = P+2 table only).
- * nk_jit_compile_check: compile the Helmholtz kernel for `nmodes` without loading it (needs NO GPU): NVRTC's wall time in
- * ms and the cubin size.  nk_jit_stats: kernels specialised for launching so far in this process and their compile time. */
+ * Kernels are prebuilt for Q = P+2 (hex P1..P10, tet / prism P1..P8).  What falls outside is compiled by NVRTC on first
+ * use from the kernel sources embedded in libnk.so, loaded through the driver API and cached per device; libnvrtc and
+ * libcuda are dlopen'ed (no link-time dependency), and a failure surfaces as NK_ERR_UNSUPPORTED at apply time.
+ *  - Reference-matrix kernels (one number, the modes per element): csrc/nk_dense.cuh for a mode count outside the
+ *    prebuilt table (tets P1..P8, trilinear hexes); cached per (device, modes, operator).
+ *  - Sum-factorised kernels: nk_basis_create accepts ANY (shape, P, Q) with 1 <= P <= 10 and P+1 <= Q <= 12 whose basis
+ *    tables fit the 32 KB kernel-parameter space (every hex; tets and prisms up to P = 9): nk_kernel<shape, P, deformed,
+ *    operator, Q> is instantiated per first use with the launch rules of the prebuilt table (they depend on Q); cached
+ *    per (device, shape, P, Q, deformed, operator).  Every operator of this header works on such a basis.
+ * nk_jit_compile_check: compile the reference-matrix Helmholtz kernel for `nmodes` without loading it (needs NO GPU):
+ * NVRTC's wall time in ms and the cubin size.  nk_jit_compile_check_kernel: the same for one sum-factorised
+ * instantiation (op: 0 bwdtrans, 1 iprod, 2 physderiv, 3 iprod_deriv, 4 mass, 5 laplacian, 6 helmholtz, 7 helmholtz on
+ * fields).  nk_jit_stats: kernels specialised for launching so far in this process and their compile time. */
 nk_status nk_jit_compile_check(int nmodes, double* compile_ms, size_t* cubin_bytes);
+nk_status nk_jit_compile_check_kernel(nk_shape shape, int P, int Q, int deformed, int op, double* compile_ms, size_t* cubin_bytes);
 nk_status nk_jit_stats(int64_t* kernels, double* compile_ms);
 
 /* ---- diagnostics ----------------------------------------------------------------------------- */

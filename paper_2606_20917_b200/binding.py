@@ -53,6 +53,7 @@ _SIG = {
     "nk_assembled_helmholtz_apply_static": (_i, [_p, _p, _p, _d, _p, _p, _p]),
     "nk_cg_solve": (_i, [_p, _p, _p, _d, _p, _p, _i, _d, _i, C.POINTER(_i), C.POINTER(_d), _p]),
     "nk_jit_compile_check": (_i, [_i, C.POINTER(_d), C.POINTER(_sz)]),
+    "nk_jit_compile_check_kernel": (_i, [_i, _i, _i, _i, _i, C.POINTER(_d), C.POINTER(_sz)]),
     "nk_jit_stats": (_i, [C.POINTER(_i64), C.POINTER(_d)]),
     "nk_set_affine_simplex_form": (_i, [_i]),
     "nk_get_affine_simplex_form": (_i, []),
@@ -358,6 +359,13 @@ def jit_compile_check(nmodes):
     """(compile ms, cubin bytes) of the NVRTC specialisation of the reference-matrix Helmholtz kernel; needs no GPU."""
     ms, nb = _d(), _sz()
     _check(lib.nk_jit_compile_check(int(nmodes), C.byref(ms), C.byref(nb)))
+    return ms.value, nb.value
+
+
+def jit_compile_check_kernel(shape, P, Q, deformed, op):
+    """NVRTC-compiles one sum-factorised instantiation without loading it (no GPU needed): (ms, cubin bytes)."""
+    ms, nb = _d(), _sz()
+    _check(lib.nk_jit_compile_check_kernel(int(shape), int(P), int(Q), int(bool(deformed)), int(op), C.byref(ms), C.byref(nb)))
     return ms.value, nb.value
 
 

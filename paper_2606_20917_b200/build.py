@@ -72,6 +72,13 @@ def build(force=False, jobs=None, verbose=False, extra_defs=(), lib=None, objdir
     if not os.path.exists(src_inc) or open(src_inc).read() != text:
         with open(src_inc, "w") as f:
             f.write(text)
+    # the same for the sum-factorised kernel template and the stage files it includes: {name, text} pairs
+    sf_inc = os.path.join(OBJ, "nk_sumfac_src.inc")
+    names = ["nk_kernels.cuh", "nk_kernel_body.cuh"] + sorted(f for f in os.listdir(CSRC) if f.startswith("nk_stage_") and f.endswith(".inc"))
+    text = "".join('{"%s", R"NKSRC(%s)NKSRC"},\n' % (n, open(os.path.join(CSRC, n)).read()) for n in names)
+    if not os.path.exists(sf_inc) or open(sf_inc).read() != text:
+        with open(sf_inc, "w") as f:
+            f.write(text)
     jit_o = os.path.join(OBJ, "nk_jit.o")
     tasks.append((jit_o, [nvcc, *COMMON, *ARCH, "-I", OBJ, "-c", os.path.join(CSRC, "nk_jit.cu"), "-o", jit_o]))
     sol_o = os.path.join(OBJ, "nk_solver.o")

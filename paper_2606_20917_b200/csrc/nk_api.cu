@@ -92,6 +92,11 @@ nk_status ensure_device()
 struct nk_basis {
     nk::HostTables t;
     const nk::InstInfo* inst = nullptr;
+    // (shape, P, Q) outside the prebuilt table: the kernels are specialised at run time (csrc/nk_jit.cu); `inst` then
+    // points at own_inst, which carries the interleave widths but no launch functions
+    bool jit = false;
+    nk::JitInfo jinfo;
+    nk::InstInfo own_inst;
     std::vector<double> tabs_flat; // DenseTabs<nm,Q> in declaration order
     std::vector<double> sx_flat;   // SimplexTabs in declaration order (simplices only)
     std::vector<double> kron[3];   // hex: the 1-D matrices M, K, C of the coefficient-space forms (NK_TAB_KRON)
@@ -150,7 +155,8 @@ bool use_dense(const nk_basis* b, int deformed, int op, nk_status* st)
     if (form == 2) return true;
     const int shape = b->t.shape, P = b->t.P;
     const bool faster = shape == nk::TET || (shape == nk::PRISM && P <= 3) || (shape == nk::HEX && P == 1);
-    return faster && nk::dense_supported(b->t.Nm);
+    // tets outside the prebuilt table (P = 9, run-time specialised basis): the reference-matrix kernel is specialised too
+    return faster && (nk::dense_supported(b->t.Nm) || (b->jit && shape == nk::TET));
 }
 } // namespace
 
@@ -175,11 +181,16 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
     if (!out) return fail(NK_ERR_INVALID_ARG, "nk_basis_create: out is NULL");
     *out = nullptr;
     if ((int)shape < 0 || (int)shape > 2 || P < 1 || Q < 2) return fail(NK_ERR_INVALID_ARG, "nk_basis_create: bad shape/P/Q");
-    InstGetter get = inst_getter((int)shape, P);
-    if (!get || Q != P + 2) {
-        char buf[160];
-        snprintf(buf, sizeof buf, "nk_basis_create: (shape=%d,P=%d,Q=%d) not instantiated (Q must be P+2; hex P<=10, tet/prism P<=8)", (int)shape, P, Q);
-        return fail(NK_ERR_UNSUPPORTED, buf);
+    InstGetter get = (Q == P + 2) ? inst_getter((int)shape, P) : nullptr;
+    nk::JitInfo jinfo;
+    if (!get) {
+        // outside the prebuilt table (Q = P+2; hex P <= 10, tet / prism P <= 8): specialised at run time on first use
+        std::string why;
+        if (!nk::sumfac_jit_info((int)shape, P, Q, &jinfo, &why)) {
+            char buf[128];
+            snprintf(buf, sizeof buf, "nk_basis_create: (shape=%d,P=%d,Q=%d) is neither prebuilt nor specialisable: ", (int)shape, P, Q);
+            return fail(NK_ERR_UNSUPPORTED, buf + why);
+        }
     }
     nk_basis* b = new (std::nothrow) nk_basis;
     if (!b) return fail(NK_ERR_ALLOC, "nk_basis_create: out of memory");
@@ -187,7 +198,23 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
         delete b;
         return fail(NK_ERR_INVALID_ARG, "nk_basis_create: table construction failed");
     }
-    b->inst = get();
+    if (get) {
+        b->inst = get();
+    } else {
+        b->jit = true;
+        b->jinfo = jinfo;
+        nk::InstInfo& oi = b->own_inst;
+        std::memset(&oi, 0, sizeof oi);
+        oi.shape = (int)shape; oi.P = P; oi.Q = Q;
+        for (int d = 0; d < 2; ++d) {
+            oi.E[d] = jinfo.E[d];
+            oi.threads[d] = jinfo.op[d][nk::OP_HELM].threads;
+            oi.blocks_per_sm_hint[d] = jinfo.op[d][nk::OP_HELM].minb;
+            oi.smem_grid[d] = jinfo.op[d][nk::OP_HELM].smem;
+        }
+        for (int k = 0; k < nk::OP_COUNT; ++k) oi.E_op_affine[k] = jinfo.op[0][k].E;
+        b->inst = &oi;
+    }
     const nk::HostTables& t = b->t;
     const int nm = t.nm;
     // DenseTabs: Ba[3][Q*nm], BaT[3][nm*Q], KM[3][4][nm*nm], D[3][Q*Q], DT[3][Q*Q], w[3][Q], aux[7][Q]
@@ -582,6 +609,13 @@ nk_status run_op(int op, const char* name, const nk_basis* b, const nk_geom* g, 
     a.g0 = (int)group0;
     a.grid_groups = (int)(group_count < 0 ? ngroups : group_count);
     if (a.g0 < 0 || a.g0 + (int64_t)a.grid_groups > ngroups) return fail(NK_ERR_INVALID_ARG, std::string(name) + ": bad group range");
+    if (b->jit) {
+        std::string why;
+        if (!nk::sumfac_jit_launch(b->jinfo, def, op, b->tabs_flat.data(), b->sx_flat.data(), a, g_num_sms, (cudaStream_t)stream, &why))
+            return fail(NK_ERR_UNSUPPORTED, std::string(name) + ": run-time specialisation failed: " + why);
+        { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
+        return NK_OK;
+    }
     cudaError_t e = b->inst->fn[def][op](b->tabs_flat.data(), b->sx_flat.data(), a, g_num_sms, (cudaStream_t)stream);
     if (e != cudaSuccess) return cuda_fail(e, name);
     { std::lock_guard<std::mutex> lk(g_mutex); ++g_launches; }
@@ -831,6 +865,12 @@ extern "C" nk_status nk_jit_compile_check(int nmodes, double* compile_ms, size_t
     if (nmodes < 1 || nmodes > 1024) return fail(NK_ERR_INVALID_ARG, "nk_jit_compile_check: 1 <= nmodes <= 1024");
     std::string why;
     if (!nk::dense_jit_compile_check(nmodes, nk::DENSE_HELM, compile_ms, cubin_bytes, &why)) return fail(NK_ERR_UNSUPPORTED, why);
+    return NK_OK;
+}
+extern "C" nk_status nk_jit_compile_check_kernel(nk_shape shape, int P, int Q, int deformed, int op, double* compile_ms, size_t* cubin_bytes)
+{
+    std::string why;
+    if (!nk::sumfac_jit_compile_check((int)shape, P, Q, deformed, op, compile_ms, cubin_bytes, &why)) return fail(NK_ERR_UNSUPPORTED, why);
     return NK_OK;
 }
 extern "C" nk_status nk_jit_stats(int64_t* kernels, double* compile_ms)

@@ -56,14 +56,14 @@ __device__ __forceinline__ void cp_async_wait_group()
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-template <int SHAPE, int P, int DEF, int OPX>
-__global__ void __launch_bounds__(TuneOp<SHAPE, P, DEF, OPX>::NT, TuneOp<SHAPE, P, DEF, OPX>::MINB)
-nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
-          const __grid_constant__ typename SimplexTabsFor<SHAPE, P + 1, P + 2>::type st, const __grid_constant__ KArgs a)
+template <int SHAPE, int P, int DEF, int OPX, int QQ = P + 2>
+__global__ void __launch_bounds__(TuneOp<SHAPE, P, DEF, OPX, QQ>::NT, TuneOp<SHAPE, P, DEF, OPX, QQ>::MINB)
+nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
+          const __grid_constant__ typename SimplexTabsFor<SHAPE, P + 1, QQ>::type st, const __grid_constant__ KArgs a)
 {
-    using T = TuneOp<SHAPE, P, DEF, OPX>;
+    using T = TuneOp<SHAPE, P, DEF, OPX, QQ>;
     constexpr int OP = (OPX == OP_HELMF) ? OP_HELM : OPX;
-    constexpr int NM = P + 1, Q = P + 2, E = T::E, LS = T::LS, LQ = T::LQ;
+    constexpr int NM = P + 1, Q = QQ, E = T::E, LS = T::LS, LQ = T::LQ;
     constexpr int NQ = Q * Q * Q, NQP = T::NQP, NMODES = k_num_modes(SHAPE, NM);
     constexpr bool IN_COEFF = (OP == OP_BWD || OP == OP_MASS || OP == OP_LAP || OP == OP_HELM);
     constexpr bool OUT_COEFF = (OP != OP_BWD && OP != OP_PHYSDERIV);
@@ -76,7 +76,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, P + 2, SHAPE == K_HEX> tabs,
     constexpr bool MASS_KRON = T::MASS_KRON;           // nk_stage_masskron.inc
     constexpr bool LAP_KRON = T::LAP_KRON;             // nk_stage_lapkron.inc
     constexpr bool KRON = T::KRON;
-    constexpr int EG = Tune<SHAPE, P, DEF>::E;         // interleave width of the geometry stream
+    constexpr int EG = Tune<SHAPE, P, DEF, QQ>::E;         // interleave width of the geometry stream
 
     extern __shared__ double sm[];
     // thread = (e, slot) over the whole block

@@ -20,10 +20,21 @@
 //     Q^3*E doubles are reused by a static plan (cf. the buffer-reuse pass);
 //     quadrature-point data never goes to HBM.
 #pragma once
+#ifndef __CUDACC_RTC__
 #include <cuda_runtime.h>
 #include <stdint.h>
 
 #include <type_traits>
+#else
+// NVRTC (run-time specialisation, csrc/nk_jit.cu) has no host headers: the one std type this file uses
+namespace std {
+template <class T, T v>
+struct integral_constant {
+    static constexpr T value = v;
+    using value_type = T;
+};
+} // namespace std
+#endif
 
 namespace nk {
 
@@ -37,16 +48,19 @@ __host__ __device__ constexpr int k_num_modes(int shape, int nm)
     return shape == K_HEX ? nm * nm * nm : shape == K_TET ? nm * (nm + 1) * (nm + 2) / 6 : nm * nm * (nm + 1) / 2;
 }
 
-// ---- launch configuration per (shape, P, deformed); Q = P+2 -----------------------------
+// ---- launch configuration per (shape, P, deformed, Q) ------------------------------------
+// QQ = points per direction.  The prebuilt table (nk_inst.cu) holds QQ = P+2, the default; any other NM <= QQ <= 12 is
+// specialised at run time (csrc/nk_jit.cu) with the rules below, which depend on Q rather than on P.
 // E  = elements per group (interleave width), LS = line slots, threads = E*LS,
 // LQ = padded length of an i-line in the point arrays (odd when E < 16 so that the
 //      (j,k)-line pass stays bank-conflict-free), MINB = blocks per SM asked of ptxas.
 // Values from the round-1 sweeps on B200 (profiles/r1_notes.md): deformed (HBM-bound) kernels want small
 // blocks (about 150-200 threads) at up to 96 registers, many of them per SM; affine (issue / shared-memory
 // bound) kernels want 72 registers and as many resident threads as that allows.
-template <int SHAPE, int P, int DEF>
+template <int SHAPE, int P, int DEF, int QQ = P + 2>
 struct Tune {
-    static constexpr int Q = P + 2;
+    static constexpr int Q = QQ;
+    static_assert(QQ >= P + 1, "a quadrature line must hold at least P+1 points (the on-chip arrays are sized by Q)");
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
@@ -59,8 +73,8 @@ struct Tune {
     // On simplices the triangular stages give every WARP one (s) or (p) value, so that the psi^b entries are
     // warp-uniform constant-bank operands; LS is rounded up to what those stages need.
     static constexpr int NM = P + 1, SPW = 32 / E;          // SPW = line slots per warp
-    static constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
-    static constexpr int warps_s1_tet()
+    __host__ __device__ static constexpr int cdiv(int a, int b) { return (a + b - 1) / b; }
+    __host__ __device__ static constexpr int warps_s1_tet()
     {
         int w = 0;
         for (int s = 0; s < NM; ++s) w += cdiv(s + 1, SPW);
@@ -130,9 +144,9 @@ struct Tune {
 // Per-operator launch configuration.  Only the affine-hex mass operator in coefficient space
 // (nk_stage_masskron.inc) departs from Tune: it has nm^2 lines of nm entries, no quadrature-point arrays, and
 // is bandwidth-bound, so it takes more elements per block (its own E; the geometry stream keeps Tune's E).
-template <int SHAPE, int P, int DEF, int OPX>
-struct TuneOp : Tune<SHAPE, P, DEF> {
-    using B = Tune<SHAPE, P, DEF>;
+template <int SHAPE, int P, int DEF, int OPX, int QQ = P + 2>
+struct TuneOp : Tune<SHAPE, P, DEF, QQ> {
+    using B = Tune<SHAPE, P, DEF, QQ>;
     static constexpr bool AFF_HEX = (SHAPE == K_HEX && !DEF);
     static constexpr bool MASS_KRON = AFF_HEX && OPX == OP_MASS;                                   // nk_stage_masskron.inc
 #if defined(NK_NO_LAPKRON)
@@ -186,7 +200,7 @@ struct TuneOp : Tune<SHAPE, P, DEF> {
 #if defined(NK_TUNE_MINB)
     static constexpr bool TET48 = false;
 #else
-    static constexpr bool TET48 = SHAPE == K_TET && !DEF && P == 4 && B::E == 4 && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
+    static constexpr bool TET48 = SHAPE == K_TET && !DEF && P == 4 && QQ == 6 && B::E == 4 && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
 #endif
     static constexpr int MINB = KRON ? (MINB_k < 1 ? 1 : MINB_k) : TET48 ? 8 : B::MINB;
 };

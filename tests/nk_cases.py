@@ -10,10 +10,11 @@ from workloads import synthetic as wl
 _ELS = {}
 
 
-def element(shape, P):
-    key = (shape, P)
+def element(shape, P, Q=None):
+    Q = P + 2 if Q is None else Q
+    key = (shape, P, Q)
     if key not in _ELS:
-        _ELS[key] = o.Element(shape, P, P + 2)
+        _ELS[key] = o.Element(shape, P, Q)
     return _ELS[key]
 
 
