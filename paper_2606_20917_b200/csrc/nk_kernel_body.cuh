@@ -56,37 +56,6 @@ __device__ __forceinline__ void cp_async_wait_group()
     asm volatile("cp.async.wait_group %0;" ::"n"(N) : "memory");
 }
 
-// ---- TMA plane ring (Tune::TRING): 1-D bulk copies global -> shared completing on an mbarrier (SASS: UBLKCP, SYNCS) ----
-__device__ __forceinline__ unsigned smem_u32(const void* p) { return (unsigned)__cvta_generic_to_shared(p); }
-__device__ __forceinline__ void tr_init(unsigned long long* bar, unsigned count)
-{
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
-}
-__device__ __forceinline__ void tr_expect_tx(unsigned long long* bar, unsigned bytes)
-{
-    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
-}
-__device__ __forceinline__ void tr_bulk_g2s(void* smem_dst, const void* gsrc, unsigned bytes, unsigned long long* bar)
-{
-    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(smem_u32(smem_dst)),
-                 "l"(gsrc), "r"(bytes), "r"(smem_u32(bar))
-                 : "memory");
-}
-// The poll is a C++ loop around ONE try_wait so that ptxas sees its structure (a label loop inside the asm text left the
-// lanes of a warp free to run ahead of a lane they depended on and spin: a hang on B200 once several blocks shared an SM).
-// Every blocking wait in the kernel is executed by whole warps for something ANOTHER warp or the copy engine produces.
-__device__ __forceinline__ void tr_wait(unsigned long long* bar, unsigned parity)
-{
-    unsigned ok;
-    do {
-        asm volatile("{\n.reg .pred p;\nmbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\nselp.u32 %0, 1, 0, p;\n}" : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity) : "memory");
-    } while (!ok);
-}
-__device__ __forceinline__ void tr_arrive(unsigned long long* bar)
-{
-    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
 template <int SHAPE, int P, int DEF, int OPX, int QQ = P + 2>
 __global__ void __launch_bounds__(TuneOp<SHAPE, P, DEF, OPX, QQ>::NT, TuneOp<SHAPE, P, DEF, OPX, QQ>::MINB)
 nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
@@ -119,13 +88,6 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
     double* __restrict__ Z = S0 + (size_t)(T::KRON ? 1 : 2) * NQP * E;
     double* __restrict__ RG = S0 + (size_t)3 * NQP * E;      // geometry ring [RING][7][threads] (T::RING > 0 only)
     (void)RG;
-    // TMA plane ring (T::TRING > 0 only): TG[slot][7][Q*Q*E], then the mbarriers full[TRING], empty[TRING]
-    constexpr int TR = T::TRING, TPL = Q * Q * E;            // TPL = doubles of one component of one k-plane of the group
-    constexpr int TR_WARPS = (TPL + 31) / 32;                // warps that hold pass-C lines (they release the slots)
-    double* __restrict__ TG = S0 + (size_t)3 * NQP * E;
-    unsigned long long* tr_full = reinterpret_cast<unsigned long long*>(TG + (size_t)TR * 7 * TPL);
-    unsigned long long* tr_empty = tr_full + TR;
-    (void)TG; (void)tr_full; (void)tr_empty; (void)TR_WARPS;
     const int e = tid % E, slot = tid / E;
     constexpr bool active = true;
 #define NK_SYNC() __syncthreads()
@@ -174,24 +136,6 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
                     const long long cnt = (a.nelem - e0 < E) ? (a.nelem - e0) : E;
                     const unsigned bytes = (unsigned)(cnt * NIN * sizeof(double)) & ~15u;
                     if (bytes && (reinterpret_cast<size_t>(base + e0 * NIN) & 15) == 0) l2_prefetch(base + e0 * NIN, bytes);
-                }
-            }
-        }
-        if constexpr (TR > 0) {
-            static_assert(TR == 0 || (LS >= Q * Q && (TPL % 2) == 0 && TPL >= 32), "the plane ring assumes one pass-C line per thread, 16-byte planes and a full first warp");
-            // thread 0 sets the barriers up and requests the first TR planes; the barrier in front of S1 publishes the set-up
-            if (tid == 0) {
-                NK_UNROLL for (int r = 0; r < TR; ++r) {
-                    tr_init(&tr_full[r], 1);
-                    tr_init(&tr_empty[r], TR_WARPS);
-                }
-                asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-                asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
-                const double* gsrc = a.geom + (size_t)g * NCG * NQ * E;
-                NK_UNROLL for (int r = 0; r < TR; ++r) {
-                    tr_expect_tx(&tr_full[r], 7u * TPL * (unsigned)sizeof(double));
-                    NK_UNROLL for (int c = 0; c < 7; ++c)
-                        tr_bulk_g2s(TG + (size_t)(r * 7 + c) * TPL, gsrc + ((size_t)c * NQ + (size_t)r * Q * Q) * E, TPL * (unsigned)sizeof(double), &tr_full[r]);
                 }
             }
         }

@@ -95,39 +95,22 @@ struct Tune {
     // RING: depth (in k-planes) of the per-thread geometry ring of the deformed Laplacian / Helmholtz kernels
     // (nk_stage_mid.inc, pass C): the 7 metric entries of the thread's next RING points are copied global -> shared
     // by cp.async while the thread works, the first RING planes from kernel entry on.  0 = plain __ldg in pass C.
-    // TRING: depth (in k-planes) of the TMA plane ring of the deformed Laplacian / Helmholtz kernels: the 7 metric entries of
-    // WHOLE k-planes of the group ([7][Q*Q*E] doubles, 7 contiguous ranges of the geometry stream) are copied global ->
-    // shared by cp.async.bulk with mbarrier completion, the first TRING planes at kernel entry (they land while the basis
-    // stages run), plane k + TRING into the slot of plane k once every warp has released it.  Bytes in flight no longer
-    // depend on resident threads or registers, and pass C issues 7 LDS per point in place of 7 LDG (no LDGSTS, unlike
-    // RING).  Excludes RING and EARLY.
-#if defined(NK_TUNE_TRING)
-    static constexpr int TRING = DEF ? (NK_TUNE_TRING < Q ? NK_TUNE_TRING : Q) : 0;
-#else
-    static constexpr int TRING = 0;
-#endif
-#if defined(NK_TUNE_TRFILL)
-    static constexpr bool TRFILL = NK_TUNE_TRFILL != 0;   // 0: only the first TRING planes come through the ring, the rest by __ldg
-#else
-    static constexpr bool TRFILL = true;
-#endif
-    static constexpr size_t smem_tring = TRING > 0 ? (size_t)TRING * 7 * Q * Q * E * sizeof(double) + 2 * TRING * sizeof(unsigned long long) : 0;
 #if defined(NK_TUNE_RING)
-    static constexpr int RING = (DEF && TRING == 0) ? (NK_TUNE_RING < Q ? NK_TUNE_RING : Q) : 0;
+    static constexpr int RING = DEF ? (NK_TUNE_RING < Q ? NK_TUNE_RING : Q) : 0;
 #else
     // B200 sweep (profiles/r2_notes.md): the ring costs 7 LDGSTS + 7 LDS per point instead of 7 LDG and loses wherever the
     // L2 prefetch alone keeps pass C fed (hexes at every order: cfg2 49.0 -> 42.8; simplices up to Q = 9: cfg5 19.5 -> 16.3);
     // it wins on the simplices at Q = 10 (cfg5:8 10.2 -> 11.6 GDoF/s), where few warps are resident to hide the L2 latency
-    static constexpr int RING = (DEF && TRING == 0 && SHAPE != K_HEX && Q >= 10) ? 2 : 0;
+    static constexpr int RING = (DEF && SHAPE != K_HEX && Q >= 10) ? 2 : 0;
 #endif
     static constexpr size_t smem_ring = (size_t)NT * RING * 7 * sizeof(double);
     // EARLY: number of k-planes of the thread's pass-C line whose 7 metric entries are requested BEFORE the barrier in
     // front of pass C (registers held across it), so that their L2 latency overlaps the wait at the barrier
     // (nk_stage_mid.inc; B200 sweep in profiles/r2_notes.md section 7)
 #if defined(NK_TUNE_EARLY)
-    static constexpr int EARLY = (DEF && RING == 0 && TRING == 0) ? (NK_TUNE_EARLY < Q ? NK_TUNE_EARLY : Q) : 0;
+    static constexpr int EARLY = (DEF && RING == 0) ? (NK_TUNE_EARLY < Q ? NK_TUNE_EARLY : Q) : 0;
 #else
-    static constexpr int EARLY = (DEF && RING == 0 && TRING == 0) ? (SHAPE != K_HEX ? 1 : Q == 9 ? 2 : 0) : 0;
+    static constexpr int EARLY = (DEF && RING == 0) ? (SHAPE != K_HEX ? 1 : Q == 9 ? 2 : 0) : 0;
 #endif
     // COLS: form of the 1-D contractions (contract below): input-outermost over the transposed tables
 #if defined(NK_TUNE_COLS)
@@ -152,7 +135,7 @@ struct Tune {
     static constexpr int REGS = DEF ? (SHAPE == K_HEX ? (Q == 4 ? 64 : (Q == 7 || Q == 10) ? 80 : 96) : (Q == 6 || Q == 8) ? 64 : 72)
                                     : Q <= 6 ? 56 : 64;
 #endif
-    static constexpr int MINB_smem = (int)((227 * 1024) / (smem_grid + smem_ring + smem_tring + 1024));
+    static constexpr int MINB_smem = (int)((227 * 1024) / (smem_grid + smem_ring + 1024));
     static constexpr int MINB_reg = 65536 / (NT * REGS);
     static constexpr int MINB = MINB_smem < 1 ? 1 : (MINB_smem < MINB_reg ? MINB_smem : (MINB_reg < 1 ? 1 : MINB_reg));
 #endif
@@ -205,10 +188,7 @@ struct TuneOp : Tune<SHAPE, P, DEF, QQ> {
     static constexpr int NT = KRON ? E * LS : B::NT;
     static constexpr bool USE_RING = B::RING > 0 && DEF && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
     static constexpr int RING = USE_RING ? B::RING : 0;
-    static constexpr bool USE_TRING = B::TRING > 0 && DEF && (OPX == OP_LAP || OPX == OP_HELM || OPX == OP_HELMF);
-    static constexpr int TRING = USE_TRING ? B::TRING : 0;
-    static constexpr size_t smem_grid = KRON ? (size_t)NARR * NQP * E * sizeof(double)
-                                             : B::smem_grid + (USE_RING ? B::smem_ring : 0) + (USE_TRING ? B::smem_tring : 0);
+    static constexpr size_t smem_grid = KRON ? (size_t)NARR * NQP * E * sizeof(double) : B::smem_grid + (USE_RING ? B::smem_ring : 0);
 #if defined(NK_TUNE_REGSK)
     static constexpr int REGSK = NK_TUNE_REGSK;
 #else
