@@ -24,7 +24,8 @@ METRIC = "Helmholtz apply GDoF/s (fp64)"
 HBM_FALLBACK_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
 FP64_NOMINAL_TFLOPS = 37.2     # 148 SM x 64 DFMA/clk x 2 x 1.965 GHz
 PER_WORKLOAD_DEFAULT = ("cfg3", "cfg3:7", "cfg3:8", "cfg5", "cfg5:8", "cfg4:1", "cfg4:4", "cfg4:7", "cfg4:10",
-                        "cfg2:7", "cfg2:10", "cfg1", "cg")
+                        "cfg2:7", "cfg2:10", "cfg2:4:7", "cfg5:5:8", "cfg1", "cg")
+# cfg2:4:7 and cfg5:5:8 run on kernels specialised at run time by NVRTC (Q = P+3: outside the prebuilt Q = P+2 table)
 
 
 def parse_args():
@@ -598,6 +599,12 @@ def main():
             except Exception as ex:
                 pw[name] = {"error": str(ex)[:200]}
         roof["per_workload"] = pw
+        try:
+            k, cms = nk.jit_stats()
+            roof["run_time_specialisation"] = {"kernels_compiled": int(k), "nvrtc_ms_total": cms,
+                                               "note": "kernels outside the prebuilt Q = P+2 table (cfgN:P:Q entries), NVRTC on first use"}
+        except Exception:
+            pass
         roof["per_workload_note"] = ("each entry: W >= 3 warm-ups, `steps` launches between two CUDA events, 4 rotating "
                                      "buffer sets; frac = algorithmic bytes (hbm) or SURVEY 8(d) flops (alu) over the measured peak; "
                                      "fp64_frac_running_form counts the flops of the coefficient-space form that runs")

@@ -100,3 +100,26 @@ def test_unsupported_triples_are_refused(nk):
         with pytest.raises(nk.NkError) as ei:
             nk.Basis(shape, P, Q)
         assert ei.value.code == 2      # NK_ERR_UNSUPPORTED
+
+
+def test_hp_mixed_batch_in_one_call(nk):
+    """SURVEY 8(f) item 2, second half: a batch whose blocks differ in shape, order, quadrature order and geometry kind, as in
+    hp-adaptivity, applied by ONE nk_helmholtz_apply_blocks call -- prebuilt sum-factorised, Kronecker, reference-matrix
+    (DMMA) and run-time specialised kernels side by side on forked streams; every block against the oracle."""
+    lam = 2.5
+    spec = [(o.HEX, 2, 4, True, 3), (o.HEX, 5, 7, False, 2), (o.TET, 3, 5, True, 2), (o.PRISM, 4, 7, True, 2),
+            (o.TET, 6, 8, False, 2), (o.HEX, 3, 6, True, 2), (o.PRISM, 1, 3, False, 3)]
+    blocks, refs = [], []
+    for i, (shape, P, Q, deformed, n) in enumerate(spec):
+        el = K.element(shape, P, Q)
+        A, J = K.geometry(shape, P, n, deformed, xi=el.xi)
+        basis = nk.Basis(shape, P, Q)
+        geom = nk.Geom(basis, A.cuda(), J.cuda(), deformed)
+        x = wl.coefficients(wl.SEED0 + 40 + i, J.shape[0], el.Nm)
+        y = torch.full_like(x, float("nan")).cuda()
+        blocks.append((basis, geom, x.cuda(), y))
+        refs.append(o.helmholtz(el, A.numpy(), J.numpy(), lam, x.numpy()))
+    nk.helmholtz_apply_blocks(blocks, lam)
+    torch.cuda.synchronize()
+    for (shape, P, Q, deformed, n), (b, g, x, y), ref in zip(spec, blocks, refs):
+        assert K.normwise_err(y.cpu().numpy(), ref) <= TOL, (shape, P, Q, deformed)
