@@ -346,6 +346,44 @@ def measure_cg(nk, dev, barrier):
     return out
 
 
+def measure_cg_partitioned(nk, dev, rank, world, barrier):
+    """The assembled Helmholtz system of config 2's mesh (32^3 deformed hexes, P4) split over the ranks by elements
+    (workloads.assembly.partition_l2g) and solved by nk_part_cg_solve: every rank applies the fused kernel to its
+    elements, the dofs on the cuts are summed by an NCCL all-reduce of the interface vector, dot products by scalar
+    all-reduces (include/nk.h).  Strong scaling of ONE system; wall clock around the solve, max over ranks."""
+    import torch
+    import torch.distributed as dist
+    from workloads import assembly as asm
+    from workloads import synthetic as wl
+    n, P, lam = 32, 4, 1.0
+    basis = nk.Basis(0, P)
+    l2g, ng = asm.hex_l2g(n, P)
+    p = asm.partition_l2g(l2g, ng, world)[rank]
+    del l2g
+    lo, hi = p["range"]
+    v0, E = wl.hex_mesh(n, device=dev)
+    A, J = wl.sinusoidal_factors(v0[lo:hi].contiguous(), E[lo:hi].contiguous(), basis.points().to(dev))
+    geom = nk.Geom(basis, A, J, True, streams=nk.Geom.METRIC)
+    del A, J
+    gs = nk.GatherScatter(p["l2g"], p["glob"].numel())
+    part = nk.Partition(gs, p["shared_dof"], p["shared_slot"], p["shared_mult"], p["n_interface"], nk.torch_allreduce())
+    b = wl.coefficients(wl.SEED0 + 77, 1, ng).reshape(ng)[p["glob"]].to(dev)         # consistent on the shared dofs
+    x = torch.zeros_like(b)
+    nk.part_cg_solve(basis, geom, part, lam, b, x, rtol=0.5, maxit=2, precond=nk.PRECOND_JACOBI)      # warm-up: diagonal, NCCL channels
+    x.zero_()
+    barrier()
+    t0 = time.perf_counter()
+    iters, rel = nk.part_cg_solve(basis, geom, part, lam, b, x, rtol=1e-8, maxit=20000, precond=nk.PRECOND_JACOBI)
+    torch.cuda.synchronize()
+    t = torch.tensor([time.perf_counter() - t0], dtype=torch.float64, device=dev)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return {"workload": "Jacobi-CG on the assembled system of 32^3 deformed hexes P4 (%d global dofs) split over %d rank(s)" % (ng, world),
+            "ranks": world, "elements_per_rank": hi - lo, "interface_dofs": p["n_interface"], "iterations": iters,
+            "relative_residual": rel, "ms_total": float(t.item()) * 1e3, "ms_per_iteration": float(t.item()) * 1e3 / max(iters, 1),
+            "collectives_per_iteration": "1 interface all-reduce (%d doubles) + all-reduces of 1 and 2 doubles" % p["n_interface"],
+            "note": "wall clock, max over ranks; the all-reduce is torch.distributed (NCCL) called back from nk_part_cg_solve"}
+
+
 def measure_side_workload(nk, name, dev, rank, barrier, hbm_peak, fp64_tf, budget_ms=40.0, gpu_index=0):
     """One entry of roofline.per_workload: the workload timed with the protocol of the headline (CUDA events, >= 3
     warm-ups, rotating buffers), about `budget_ms` of kernel time -- the length of the headline's own timed region
@@ -489,7 +527,8 @@ def main():
         raise SystemExit("bench.py needs a CUDA device: libnk has no CPU fallback")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
-    if world > 1:
+    under_torchrun = "RANK" in os.environ and "MASTER_ADDR" in os.environ
+    if world > 1 or under_torchrun:
         dist.init_process_group("nccl", device_id=dev)
     import paper_2606_20917_b200 as nk       # fails loudly if libnk.so is missing
     if args.form:
@@ -537,8 +576,16 @@ def main():
     if w.op == "helmholtz" and args.fields == 1:
         e2e = measure_e2e(nk, w, world, barrier, dev, args.steps)
 
+    # the one path with a data-path collective: the assembled system on a mesh split over the ranks (NCCL all-reduce)
+    cg_part = None
+    if dist.is_initialized() and args.workload == "cfg2" and args.fields == 1:
+        try:
+            cg_part = measure_cg_partitioned(nk, dev, rank, world, barrier)
+        except Exception as ex:
+            cg_part = {"error": str(ex)[:300]}
+
     if rank != 0:
-        if world > 1:
+        if dist.is_initialized():
             dist.destroy_process_group()
         return
 
@@ -618,8 +665,10 @@ def main():
             "config": config,
             "clocks": sampler.result(), "e2e": e2e, "gpu_launches": int(launches),
             "roofline": roof, "cpu_baseline": cpu_baseline}
+    if cg_part is not None:
+        line["cg_partitioned"] = cg_part
     print(json.dumps(line), flush=True)
-    if world > 1:
+    if dist.is_initialized():
         dist.destroy_process_group()
 
 

@@ -220,6 +220,39 @@ enum { NK_PRECOND_NONE = 0, NK_PRECOND_JACOBI = 1 };
 nk_status nk_cg_solve(const nk_basis* b, const nk_geom* g, const nk_gs* gs, double lambda, const double* rhs, double* x,
                       int precond, double rtol, int maxit, int* iters, double* relres, void* stream);
 
+/* ---- the same system on a mesh split over ranks (the one exchange step) --------------
+ * Elements are independent and the paper's runs give every rank a segment of elements; the ASSEMBLED
+ * system couples the segments through the dofs on the cuts.  Each rank (one process per GPU) holds its elements, an
+ * nk_gs over its OWN numbering of the dofs its elements touch, and an nk_part that lists which of those dofs other ranks
+ * hold too:
+ *   shared_dof[i]   rank-local dof (0 <= . < nk_gs_num_global), each at most once;
+ *   shared_slot[i]  its position in the interface vector of n_interface entries -- the same numbering on every rank;
+ *   shared_mult[i]  number of ranks that hold it (>= 2).
+ * Vectors are CONSISTENT: a shared dof carries the same value on every rank that holds it (rhs and the initial x on
+ * entry; x on return).  Then
+ *   nk_part_assembled_helmholtz_apply:  out = A in, A the operator of the WHOLE mesh: the rank's own Q^T (L + lambda M) Q,
+ *       then out[shared] summed over the ranks (pack into the interface vector, all-reduce, unpack);
+ *   nk_part_exchange_sum:               that sum alone, in place (e.g. to assemble a right-hand side);
+ *   nk_part_cg_solve:                   nk_cg_solve on the whole mesh: dot products weigh a shared dof by 1 / multiplicity
+ *       and are all-reduced (one all-reduce of 1 and one of 2 doubles per iteration, one interface all-reduce per
+ *       operator application); NK_PRECOND_JACOBI uses the diagonal of the whole mesh's operator.
+ * Constrained dofs (nk_gs_set_constrained) must be constrained on every rank that holds them; they are not exchanged.
+ * The all-reduce is the caller's: `allreduce(user, device_buf, n, stream)` sums n doubles at the DEVICE pointer in place
+ * over all ranks and returns 0; its work must be ordered after everything enqueued on `stream` before the call and
+ * before everything enqueued after it (run it on that stream).  The Python binding passes torch.distributed (NCCL over
+ * NVLink).  Every rank must make the same sequence of calls (they are collective); a rank without elements takes part
+ * with an nk_gs of zero elements.  Iteration counts and residuals are identical on all ranks.                      */
+typedef int (*nk_allreduce_fn)(void* user, double* device_buf, int64_t n, void* stream);
+typedef struct nk_part nk_part;
+nk_status nk_part_create(nk_gs* gs, int64_t n_shared, const int64_t* shared_dof, const int64_t* shared_slot, const int32_t* shared_mult,
+                         int64_t n_interface, nk_allreduce_fn allreduce, void* user, nk_part** out);
+nk_status nk_part_destroy(nk_part* p);
+nk_status nk_part_exchange_sum(nk_part* p, double* vec, void* stream);
+nk_status nk_part_assembled_helmholtz_apply(const nk_basis* b, const nk_geom* g, nk_part* p, double lambda, const double* in,
+                                            double* out, void* stream);
+nk_status nk_part_cg_solve(const nk_basis* b, const nk_geom* g, nk_part* p, double lambda, const double* rhs, double* x, int precond,
+                           double rtol, int maxit, int* iters, double* relres, void* stream);
+
 /* ---- form of the affine simplex operators ------------------------------------------------------
  * With constant dxi/dx and |J| the operators of Eq. 6-7 are (L + lambda M)_e = sum_{c<6} G^e_c K_c +
  * lambda |J_e| K_6 with seven Nm x Nm matrices of the STANDARD element (the quadrature sums of Eq. 7 with the chain of

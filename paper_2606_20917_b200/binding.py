@@ -52,6 +52,11 @@ _SIG = {
     "nk_static_max_local_dofs": (_i64, []),
     "nk_assembled_helmholtz_apply_static": (_i, [_p, _p, _p, _d, _p, _p, _p]),
     "nk_cg_solve": (_i, [_p, _p, _p, _d, _p, _p, _i, _d, _i, C.POINTER(_i), C.POINTER(_d), _p]),
+    "nk_part_create": (_i, [_p, _i64, _p, _p, _p, _i64, _p, _p, C.POINTER(_p)]),
+    "nk_part_destroy": (_i, [_p]),
+    "nk_part_exchange_sum": (_i, [_p, _p, _p]),
+    "nk_part_assembled_helmholtz_apply": (_i, [_p, _p, _p, _d, _p, _p, _p]),
+    "nk_part_cg_solve": (_i, [_p, _p, _p, _d, _p, _p, _i, _d, _i, C.POINTER(_i), C.POINTER(_d), _p]),
     "nk_jit_compile_check": (_i, [_i, C.POINTER(_d), C.POINTER(_sz)]),
     "nk_jit_compile_check_kernel": (_i, [_i, _i, _i, _i, _i, C.POINTER(_d), C.POINTER(_sz)]),
     "nk_jit_stats": (_i, [C.POINTER(_i64), C.POINTER(_d)]),
@@ -352,6 +357,82 @@ def cg_solve(basis, geom, gs, lam, rhs, x, rtol=1e-10, maxit=1000, precond=PRECO
     it, rel = _i(), _d()
     _check(lib.nk_cg_solve(basis.h, geom.h, gs.h, float(lam), _field(rhs, gs.nglobal, "rhs"), _field(x, gs.nglobal, "x"),
                            int(precond), float(rtol), int(maxit), C.byref(it), C.byref(rel), _stream(stream)))
+    return it.value, rel.value
+
+
+# ---- the assembled system on a mesh split over ranks (include/nk.h: nk_part_*) ----
+_ALLREDUCE_FN = C.CFUNCTYPE(C.c_int, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p)
+
+
+class _DevicePtr:
+    """a device pointer of n doubles as seen by torch.as_tensor (no copy)"""
+
+    def __init__(self, ptr, n):
+        self.__cuda_array_interface__ = {"shape": (int(n),), "typestr": "<f8", "data": (int(ptr), False), "version": 2}
+
+
+def torch_allreduce(group=None):
+    """the all-reduce of a Partition over torch.distributed (NCCL over NVLink on GPUs): sums the tensor in place"""
+    import torch.distributed as dist
+
+    def f(t):
+        dist.all_reduce(t, op=dist.ReduceOp.SUM, group=group)
+    return f
+
+
+class Partition:
+    """nk_part handle: this rank's share of a mesh split over ranks.  shared_dof / shared_slot: int64 CPU tensors,
+    shared_mult: int32 CPU tensor (workloads.assembly.partition_l2g produces them); allreduce(tensor): sums a float64 CUDA
+    tensor in place over all ranks on the current stream (torch_allreduce(), or any callable for tests)."""
+
+    def __init__(self, gs, shared_dof, shared_slot, shared_mult, n_interface, allreduce):
+        for t, dt in ((shared_dof, torch.int64), (shared_slot, torch.int64), (shared_mult, torch.int32)):
+            if t.dtype != dt or t.is_cuda or not t.is_contiguous() or t.numel() != shared_dof.numel():
+                raise ValueError("shared_dof / shared_slot: contiguous int64 host tensors, shared_mult: int32, of one length")
+
+        def cb(user, buf, n, stream):
+            try:
+                allreduce(torch.as_tensor(_DevicePtr(buf, n), device="cuda"))
+                return 0
+            except Exception:          # never let an exception cross the C boundary
+                import traceback
+                traceback.print_exc()
+                return 1
+        self._cb = _ALLREDUCE_FN(cb)   # kept alive as long as the handle
+        ns = shared_dof.numel()
+        h = _p()
+        _check(lib.nk_part_create(gs.h, ns, shared_dof.data_ptr() if ns else None, shared_slot.data_ptr() if ns else None,
+                                  shared_mult.data_ptr() if ns else None, int(n_interface), C.cast(self._cb, _p), None, C.byref(h)))
+        self.h, self.gs = h, gs
+
+    def close(self):
+        if self.h:
+            lib.nk_part_destroy(self.h)
+            self.h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def part_exchange_sum(part, vec, stream=None):
+    _check(lib.nk_part_exchange_sum(part.h, _field(vec, part.gs.nglobal, "vec"), _stream(stream)))
+
+
+def part_assembled_helmholtz_apply(basis, geom, part, lam, inp, out, stream=None):
+    gs = part.gs
+    _check(lib.nk_part_assembled_helmholtz_apply(basis.h, geom.h, part.h, float(lam), _field(inp, gs.nglobal, "in"),
+                                                 _field(out, gs.nglobal, "out"), _stream(stream)))
+
+
+def part_cg_solve(basis, geom, part, lam, rhs, x, rtol=1e-10, maxit=1000, precond=PRECOND_JACOBI, stream=None):
+    """nk_part_cg_solve: (iterations, relative residual), identical on every rank; collective."""
+    gs = part.gs
+    it, rel = _i(), _d()
+    _check(lib.nk_part_cg_solve(basis.h, geom.h, part.h, float(lam), _field(rhs, gs.nglobal, "rhs"), _field(x, gs.nglobal, "x"),
+                                int(precond), float(rtol), int(maxit), C.byref(it), C.byref(rel), _stream(stream)))
     return it.value, rel.value
 
 

@@ -443,6 +443,294 @@ extern "C" nk_status nk_cg_solve(const nk_basis* b, const nk_geom* g, const nk_g
     return NK_OK;
 }
 
+// =========================== partitioned solve (several ranks, one sub-mesh each) ===========================
+// A mesh split over ranks by elements (contiguous element ranges) shares the dofs on the cut: every
+// rank holds them in its own numbering and the assembled operator needs their contributions from all ranks.  That sum is
+// the one data-path exchange of this library ("first consumer of multi-GPU"):
+//     y = A x:   local Q^T H Q on the rank's elements, then  y[shared] <- sum over ranks  (pack, all-reduce, unpack)
+//     <a, b>:    sum_i w_i a_i b_i with w_i = 1 / (number of ranks holding dof i), then a scalar all-reduce
+// for vectors that are CONSISTENT (equal on every rank that holds a dof).  The all-reduce itself is the caller's
+// (a C callback: torch.distributed / NCCL over NVLink in the Python binding); everything else runs in the kernels below.
+namespace {
+enum { S_TMP0 = 6, S_TMP1 = 7 };
+__global__ void pack_kernel(const int* __restrict__ sdof, const int* __restrict__ sslot, const unsigned char* __restrict__ free,
+                            const double* __restrict__ vec, double* __restrict__ ibuf, long long ns)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ns; i += (long long)gridDim.x * blockDim.x) {
+        const int d = sdof[i];
+        ibuf[sslot[i]] = (!free || free[d]) ? vec[d] : 0.0;     // constrained dofs keep their identity row: nothing to sum
+    }
+}
+__global__ void unpack_kernel(const int* __restrict__ sdof, const int* __restrict__ sslot, const unsigned char* __restrict__ free,
+                              double* __restrict__ vec, const double* __restrict__ ibuf, long long ns)
+{
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < ns; i += (long long)gridDim.x * blockDim.x) {
+        const int d = sdof[i];
+        if (!free || free[d]) vec[d] = ibuf[sslot[i]];
+    }
+}
+__global__ void __launch_bounds__(kRedThreads) dot_partial_w(const double* __restrict__ a, const double* __restrict__ b, const double* __restrict__ w,
+                                                              long long n, double* __restrict__ partial)
+{
+    double v = 0.0;
+    for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += (long long)gridDim.x * blockDim.x) v = fma(w[i] * a[i], b[i], v);
+    const double s = block_sum(v);
+    if (threadIdx.x == 0) partial[blockIdx.x] = s;
+}
+__global__ void __launch_bounds__(kRedThreads) sum_final(const double* __restrict__ partial, int nb, double* __restrict__ sc, int slot)
+{
+    double v = 0.0;
+    for (int i = threadIdx.x; i < nb; i += blockDim.x) v += partial[i];
+    const double s = block_sum(v);
+    if (threadIdx.x == 0) sc[slot] = s;
+}
+// the scalar updates of CG once the reduced sums sit in sc[S_TMP0], sc[S_TMP1]
+__global__ void cg_scalars(double* __restrict__ sc, int which)
+{
+    if (which == S_RR) {                  // start: rz, rr
+        sc[S_RR] = sc[S_TMP0];
+        sc[S_NORM2] = sc[S_TMP1];
+    } else if (which == S_PAP) {          // alpha = rz / pAp
+        sc[S_PAP] = sc[S_TMP0];
+        sc[S_ALPHA] = sc[S_TMP0] != 0.0 ? sc[S_RR] / sc[S_TMP0] : 0.0;
+    } else {                              // beta = rz_new / rz ; rz = rz_new ; rr
+        sc[S_RRNEW] = sc[S_TMP0];
+        sc[S_BETA] = sc[S_RR] != 0.0 ? sc[S_TMP0] / sc[S_RR] : 0.0;
+        sc[S_RR] = sc[S_TMP0];
+        sc[S_NORM2] = sc[S_TMP1];
+    }
+}
+} // namespace
+
+struct nk_part {
+    nk_gs* gs = nullptr;
+    int64_t ns = 0, ni = 0;
+    int *d_sdof = nullptr, *d_sslot = nullptr;
+    double *d_w = nullptr, *d_ibuf = nullptr, *d_diag = nullptr;     // weights [nglobal], interface vector [ni], exchanged diag(A)
+    const void* diag_geom = nullptr;
+    double diag_lambda = 0.0;
+    nk_allreduce_fn fn = nullptr;
+    void* user = nullptr;
+};
+
+extern "C" nk_status nk_part_destroy(nk_part* p)
+{
+    if (!p) return NK_OK;
+    for (void* q : {(void*)p->d_sdof, (void*)p->d_sslot, (void*)p->d_w, (void*)p->d_ibuf, (void*)p->d_diag})
+        if (q) cudaFree(q);
+    delete p;
+    return NK_OK;
+}
+
+extern "C" nk_status nk_part_create(nk_gs* gs, int64_t n_shared, const int64_t* shared_dof, const int64_t* shared_slot, const int32_t* shared_mult,
+                                    int64_t n_interface, nk_allreduce_fn allreduce, void* user, nk_part** out)
+{
+    if (!out) return sfail(NK_ERR_INVALID_ARG, "nk_part_create: out is NULL");
+    *out = nullptr;
+    if (!gs || !allreduce || n_shared < 0 || n_interface < 0 || n_shared > n_interface ||
+        (n_shared > 0 && (!shared_dof || !shared_slot || !shared_mult)))
+        return sfail(NK_ERR_INVALID_ARG, "nk_part_create: bad arguments");
+    std::vector<int> sd((size_t)n_shared), ss((size_t)n_shared);
+    std::vector<double> w((size_t)gs->nglobal, 1.0);
+    std::vector<unsigned char> seen((size_t)n_interface, 0);
+    for (int64_t i = 0; i < n_shared; ++i) {
+        if (shared_dof[i] < 0 || shared_dof[i] >= gs->nglobal || shared_slot[i] < 0 || shared_slot[i] >= n_interface || shared_mult[i] < 2)
+            return sfail(NK_ERR_INVALID_ARG, "nk_part_create: shared dof / slot out of range, or multiplicity < 2");
+        if (seen[(size_t)shared_slot[i]] || w[(size_t)shared_dof[i]] != 1.0)
+            return sfail(NK_ERR_INVALID_ARG, "nk_part_create: a shared dof or an interface slot is listed twice");
+        seen[(size_t)shared_slot[i]] = 1;
+        sd[(size_t)i] = (int)shared_dof[i];
+        ss[(size_t)i] = (int)shared_slot[i];
+        w[(size_t)shared_dof[i]] = 1.0 / (double)shared_mult[i];
+    }
+    nk_part* p = new (std::nothrow) nk_part;
+    if (!p) return sfail(NK_ERR_ALLOC, "nk_part_create: out of memory");
+    p->gs = gs;
+    p->ns = n_shared;
+    p->ni = n_interface;
+    p->fn = allreduce;
+    p->user = user;
+    cudaError_t e = cudaMalloc(&p->d_w, (size_t)(gs->nglobal ? gs->nglobal : 1) * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_diag, (size_t)(gs->nglobal ? gs->nglobal : 1) * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_ibuf, (size_t)(n_interface ? n_interface : 1) * sizeof(double));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_sdof, (size_t)(n_shared ? n_shared : 1) * sizeof(int));
+    if (e == cudaSuccess) e = cudaMalloc(&p->d_sslot, (size_t)(n_shared ? n_shared : 1) * sizeof(int));
+    if (e == cudaSuccess && gs->nglobal) e = cudaMemcpy(p->d_w, w.data(), (size_t)gs->nglobal * sizeof(double), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && n_shared) e = cudaMemcpy(p->d_sdof, sd.data(), (size_t)n_shared * sizeof(int), cudaMemcpyHostToDevice);
+    if (e == cudaSuccess && n_shared) e = cudaMemcpy(p->d_sslot, ss.data(), (size_t)n_shared * sizeof(int), cudaMemcpyHostToDevice);
+    if (e != cudaSuccess) {
+        const std::string msg = std::string("nk_part_create: ") + cudaGetErrorString(e);
+        nk_part_destroy(p);
+        return sfail(e == cudaErrorMemoryAllocation ? NK_ERR_ALLOC : NK_ERR_CUDA, msg);
+    }
+    *out = p;
+    return NK_OK;
+}
+
+// vec[shared] <- sum over ranks of vec[shared] (free dofs only); every rank must call it (the all-reduce is collective)
+static nk_status part_exchange(nk_part* p, double* vec, void* stream)
+{
+    if (p->ni == 0) return NK_OK;
+    cudaStream_t s = (cudaStream_t)stream;
+    cudaError_t e = cudaMemsetAsync(p->d_ibuf, 0, (size_t)p->ni * sizeof(double), s);
+    if (e != cudaSuccess) return sfail(NK_ERR_CUDA, std::string("partition exchange: ") + cudaGetErrorString(e));
+    if (p->ns > 0) {
+        pack_kernel<<<grid_for(p->ns), 256, 0, s>>>(p->d_sdof, p->d_sslot, p->gs->d_free, vec, p->d_ibuf, p->ns);
+        nk_count_launches_(1);
+    }
+    if (p->fn(p->user, p->d_ibuf, p->ni, stream) != 0) return sfail(NK_ERR_CUDA, "partition exchange: the all-reduce callback failed");
+    if (p->ns > 0) {
+        unpack_kernel<<<grid_for(p->ns), 256, 0, s>>>(p->d_sdof, p->d_sslot, p->gs->d_free, vec, p->d_ibuf, p->ns);
+        nk_count_launches_(1);
+    }
+    e = cudaGetLastError();
+    return e == cudaSuccess ? NK_OK : sfail(NK_ERR_CUDA, std::string("partition exchange: ") + cudaGetErrorString(e));
+}
+
+static nk_status part_check(const char* name, const nk_basis* b, const nk_geom* g, const nk_part* p)
+{
+    if (!b || !g || !p) return sfail(NK_ERR_INVALID_ARG, std::string(name) + ": NULL argument");
+    if (p->gs->nelem != nk_geom_num_elements(g) || p->gs->nm != nk_basis_num_modes(b))
+        return sfail(NK_ERR_SHAPE_MISMATCH, std::string(name) + ": the map does not belong to this block");
+    return NK_OK;
+}
+
+extern "C" nk_status nk_part_exchange_sum(nk_part* p, double* vec, void* stream)
+{
+    if (!p || (!vec && p->gs->nglobal > 0)) return sfail(NK_ERR_INVALID_ARG, "nk_part_exchange_sum: NULL argument");
+    std::lock_guard<std::mutex> lk(p->gs->mu);
+    return part_exchange(p, vec, stream);
+}
+
+extern "C" nk_status nk_part_assembled_helmholtz_apply(const nk_basis* b, const nk_geom* g, nk_part* p, double lambda, const double* in,
+                                                       double* out, void* stream)
+{
+    nk_status st = part_check("nk_part_assembled_helmholtz_apply", b, g, p);
+    if (st != NK_OK) return st;
+    if (!in || !out || in == out) return sfail(NK_ERR_INVALID_ARG, "nk_part_assembled_helmholtz_apply: NULL or aliased vectors");
+    nk_gs* gs = p->gs;
+    std::lock_guard<std::mutex> lk(gs->mu);
+    st = ensure_work(gs);
+    if (st != NK_OK) return st;
+    if (gs->nglobal > 0) {
+        st = assembled_apply(b, g, gs, lambda, in, out, stream);
+        if (st != NK_OK) return st;
+    }
+    return part_exchange(p, out, stream);
+}
+
+extern "C" nk_status nk_part_cg_solve(const nk_basis* b, const nk_geom* g, nk_part* p, double lambda, const double* rhs, double* x, int precond,
+                                      double rtol, int maxit, int* iters_out, double* relres_out, void* stream)
+{
+    if (precond != NK_PRECOND_NONE && precond != NK_PRECOND_JACOBI) return sfail(NK_ERR_INVALID_ARG, "nk_part_cg_solve: unknown preconditioner");
+    nk_status st = part_check("nk_part_cg_solve", b, g, p);
+    if (st != NK_OK) return st;
+    if (!rhs || !x || rhs == x) return sfail(NK_ERR_INVALID_ARG, "nk_part_cg_solve: NULL or aliased vectors");
+    if (!(rtol >= 0.0) || maxit < 0) return sfail(NK_ERR_INVALID_ARG, "nk_part_cg_solve: rtol >= 0 and maxit >= 0 required");
+    if (iters_out) *iters_out = 0;
+    if (relres_out) *relres_out = 0.0;
+    nk_gs* gs = p->gs;
+    std::lock_guard<std::mutex> lk(gs->mu);
+    st = ensure_work(gs);
+    if (st != NK_OK) return st;
+    cudaStream_t s = (cudaStream_t)stream;
+    const long long n = gs->nglobal;        // a rank may hold no element: it still takes part in every collective
+    const int gv = grid_for(n > 0 ? n : 1);
+    double h[S_COUNT];
+    auto dotw = [&](const double* a_, const double* b_, int slot) {
+        dot_partial_w<<<kRedBlocks, kRedThreads, 0, s>>>(a_, b_, p->d_w, n, gs->d_partial);
+        sum_final<<<1, kRedThreads, 0, s>>>(gs->d_partial, kRedBlocks, gs->d_sc, slot);
+        nk_count_launches_(2);
+    };
+    auto reduce = [&](int count, int which) -> nk_status {     // all-reduce sc[S_TMP0 .. S_TMP0 + count), then the scalar updates
+        if (p->fn(p->user, gs->d_sc + S_TMP0, count, stream) != 0) return sfail(NK_ERR_CUDA, "nk_part_cg_solve: the all-reduce callback failed");
+        if (which >= 0) {
+            cg_scalars<<<1, 1, 0, s>>>(gs->d_sc, which);
+            nk_count_launches_(1);
+        }
+        return NK_OK;
+    };
+    auto read_scalars = [&]() -> nk_status {
+        cudaError_t e = cudaMemcpyAsync(h, gs->d_sc, sizeof h, cudaMemcpyDeviceToHost, s);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        return e == cudaSuccess ? NK_OK : sfail(NK_ERR_CUDA, std::string("nk_part_cg_solve: ") + cudaGetErrorString(e));
+    };
+    auto apply = [&](const double* in, double* out) -> nk_status {
+        if (n > 0) {
+            nk_status a = assembled_apply(b, g, gs, lambda, in, out, stream);
+            if (a != NK_OK) return a;
+        }
+        return part_exchange(p, out, stream);
+    };
+    const bool pc = precond == NK_PRECOND_JACOBI;
+    if (pc && !(p->diag_geom == (const void*)g && p->diag_lambda == lambda)) {
+        // diag(A) of the WHOLE mesh: the rank's own Q^T diag(H^e), summed over the ranks on the shared dofs
+        if (n > 0) {
+            st = assembled_diagonal(b, g, gs, lambda, stream);
+            if (st != NK_OK) return st;
+            cudaError_t e = cudaMemcpyAsync(p->d_diag, gs->d_diag, (size_t)n * sizeof(double), cudaMemcpyDeviceToDevice, s);
+            if (e != cudaSuccess) return sfail(NK_ERR_CUDA, "nk_part_cg_solve: copy of the diagonal");
+        }
+        st = part_exchange(p, p->d_diag, stream);
+        if (st != NK_OK) return st;
+        p->diag_geom = (const void*)g;
+        p->diag_lambda = lambda;
+    }
+    double* z = pc ? gs->d_z : gs->d_r;
+    // ||b||
+    dotw(rhs, rhs, S_TMP0);
+    st = reduce(1, -1);
+    if (st == NK_OK) st = read_scalars();
+    if (st != NK_OK) return st;
+    const double bnorm = std::sqrt(h[S_TMP0]);
+    if (!(bnorm > 0.0)) {
+        cudaError_t e = n > 0 ? cudaMemsetAsync(x, 0, (size_t)n * sizeof(double), s) : cudaSuccess;
+        if (e == cudaSuccess) e = cudaStreamSynchronize(s);
+        return e == cudaSuccess ? NK_OK : sfail(NK_ERR_CUDA, "nk_part_cg_solve: memset");
+    }
+    st = apply(x, gs->d_Ap);
+    if (st != NK_OK) return st;
+    init_rp<<<gv, 256, 0, s>>>(gs->d_r, gs->d_p, rhs, gs->d_Ap, n);
+    nk_count_launches_(1);
+    if (pc) {
+        jacobi_apply<<<gv, 256, 0, s>>>(z, gs->d_r, p->d_diag, n);
+        cudaError_t e = n > 0 ? cudaMemcpyAsync(gs->d_p, z, (size_t)n * sizeof(double), cudaMemcpyDeviceToDevice, s) : cudaSuccess;
+        if (e != cudaSuccess) return sfail(NK_ERR_CUDA, "nk_part_cg_solve: copy");
+        nk_count_launches_(1);
+    }
+    dotw(gs->d_r, z, S_TMP0);
+    dotw(gs->d_r, gs->d_r, S_TMP1);
+    st = reduce(2, S_RR);
+    if (st == NK_OK) st = read_scalars();
+    if (st != NK_OK) return st;
+    double rel = std::sqrt(h[S_NORM2]) / bnorm;
+    int it = 0;
+    while (it < maxit && rel > rtol) {          // rel is the same on every rank: all ranks leave the loop together
+        st = apply(gs->d_p, gs->d_Ap);
+        if (st != NK_OK) return st;
+        dotw(gs->d_p, gs->d_Ap, S_TMP0);
+        st = reduce(1, S_PAP);
+        if (st != NK_OK) return st;
+        update_xr<<<gv, 256, 0, s>>>(x, gs->d_r, gs->d_p, gs->d_Ap, gs->d_sc, n);
+        if (pc) jacobi_apply<<<gv, 256, 0, s>>>(z, gs->d_r, p->d_diag, n);
+        dotw(gs->d_r, z, S_TMP0);
+        dotw(gs->d_r, gs->d_r, S_TMP1);
+        st = reduce(2, S_RRNEW);
+        if (st != NK_OK) return st;
+        update_p<<<gv, 256, 0, s>>>(gs->d_p, z, gs->d_sc, n);
+        nk_count_launches_(pc ? 3 : 2);
+        st = read_scalars();
+        if (st != NK_OK) return st;
+        ++it;
+        if (!(h[S_PAP] > 0.0)) return sfail(NK_ERR_INVALID_ARG, "nk_part_cg_solve: p.Ap <= 0 (the operator is not positive definite)");
+        rel = std::sqrt(h[S_NORM2]) / bnorm;
+    }
+    if (iters_out) *iters_out = it;
+    if (relres_out) *relres_out = rel;
+    return NK_OK;
+}
+
+
 // =========================== the entry point that allocates nothing ===========================
 // nk_assembled_helmholtz_apply_static (nk.h): nk_assembled_helmholtz_apply with the two local work vectors (Q in and
 // H Q in, [nelem][Nm] each) in a file-scope device array instead of cudaMalloc'ed work space of the nk_gs handle, for

@@ -163,3 +163,136 @@ def test_solver_errors(nk):
     assert code == 1                                             # unknown preconditioner
     it, rel = nk.cg_solve(basis, geom, gs, 1.0, torch.zeros_like(x), y, rtol=1e-8, maxit=10)
     assert it == 0 and float(y.abs().max()) == 0.0               # rhs = 0 -> x = 0
+
+
+# ---- the assembled system on a mesh split over ranks (include/nk.h: nk_part_*) ----
+import threading
+
+
+def _run_ranks(world, fn):
+    """runs fn(rank) on `world` host threads (the library calls release the GIL; the all-reduce callbacks meet at a
+    barrier) and re-raises the first exception.  The ranks' KERNELS never wait for one another: each thread synchronises
+    its stream before the host-side rendezvous."""
+    err, th = [None] * world, []
+
+    def body(r):
+        try:
+            torch.cuda.set_device(0)
+            fn(r)
+        except BaseException as e:      # noqa: BLE001 -- reported in the main thread
+            err[r] = e
+    for r in range(world):
+        th.append(threading.Thread(target=body, args=(r,)))
+        th[-1].start()
+    for t in th:
+        t.join(timeout=300)
+    assert not any(t.is_alive() for t in th), "a rank did not finish"
+    for e in err:
+        if e is not None:
+            raise e
+
+
+class _HostAllreduce:
+    """in-process all-reduce over `world` threads: every rank hands in its tensor, the last one to arrive sums them in a
+    fixed order and writes the sum back to all; calls are matched by a barrier (all ranks make the same sequence)."""
+
+    def __init__(self, world):
+        self.world, self.bar, self.t, self.calls = world, threading.Barrier(world), [None] * world, 0
+
+    def make(self, rank):
+        def f(t):
+            torch.cuda.current_stream().synchronize()      # my contribution is complete
+            self.t[rank] = t
+            if self.bar.wait(timeout=120) == 0:
+                s = self.t[0].clone()
+                for k in range(1, self.world):
+                    s += self.t[k]
+                for k in range(self.world):
+                    self.t[k].copy_(s)
+                torch.cuda.synchronize()
+                self.calls += 1
+            self.bar.wait(timeout=120)
+        return f
+
+
+@pytest.mark.parametrize("world", [2, 3])
+@pytest.mark.parametrize("precond,dirichlet", [(0, False), (1, False), (1, True)])
+def test_partitioned_apply_and_cg_against_the_whole_mesh(nk, world, precond, dirichlet):
+    """a 3^3 deformed hex mesh at P3 cut into `world` element ranges (workloads.assembly.partition_l2g): the partitioned
+    operator and CG solve of every rank against the oracle's dense matrix of the WHOLE mesh and against nk_cg_solve on
+    one rank; Jacobi uses the whole mesh's diagonal; Dirichlet dofs on the cut stay fixed."""
+    n, P = 3, 3
+    lam = 0.0 if dirichlet else 1.75
+    el, A, J, basis, geom, l2g, ng = setup(nk, n, P, True)
+    G = o.assembled_matrix(el, A.numpy(), J.numpy(), lam, l2g.numpy(), ng)
+    bd = asm.hex_boundary_dofs(n, P)
+    if dirichlet:
+        G = o.constrained_matrix(G, bd.numpy())
+    rng = np.random.Generator(np.random.Philox(77 + world))
+    u, b = rng.standard_normal(ng), rng.standard_normal(ng)
+    if dirichlet:
+        b[bd.numpy()] = 0.0
+    xs = np.linalg.solve(G, b)
+    rtol = 1e-10
+    # one rank, whole mesh: the iteration count to reproduce
+    gs1 = nk.GatherScatter(l2g, ng)
+    if dirichlet:
+        gs1.set_constrained(bd)
+    x1 = torch.zeros(ng, dtype=torch.float64, device="cuda")
+    it1, _ = nk.cg_solve(basis, geom, gs1, lam, torch.from_numpy(b).cuda(), x1, rtol=rtol, maxit=20 * ng, precond=precond)
+    parts = asm.partition_l2g(l2g, ng, world)
+    assert sum(p["range"][1] - p["range"][0] for p in parts) == n ** 3 and parts[0]["n_interface"] > 0
+    comm = _HostAllreduce(world)
+    ranks = []
+    for r, p in enumerate(parts):
+        lo, hi = p["range"]
+        g_r = nk.Geom(basis, A[lo:hi].contiguous().cuda(), J[lo:hi].contiguous().cuda(), True)
+        gs_r = nk.GatherScatter(p["l2g"], p["glob"].numel())
+        if dirichlet:
+            isbd = torch.zeros(ng, dtype=torch.bool)
+            isbd[bd] = True
+            gs_r.set_constrained(torch.nonzero(isbd[p["glob"]]).reshape(-1).contiguous())
+        part = nk.Partition(gs_r, p["shared_dof"], p["shared_slot"], p["shared_mult"], p["n_interface"], comm.make(r))
+        ranks.append((g_r, gs_r, part, p["glob"].numpy()))
+    out, sol, its = [None] * world, [None] * world, [None] * world
+
+    def rank_body(r):
+        g_r, gs_r, part, glob = ranks[r]
+        y = torch.full((glob.size,), float("nan"), dtype=torch.float64, device="cuda")
+        nk.part_assembled_helmholtz_apply(basis, g_r, part, lam, torch.from_numpy(u[glob]).cuda(), y)
+        out[r] = y.cpu().numpy()
+        x = torch.zeros(glob.size, dtype=torch.float64, device="cuda")
+        its[r] = nk.part_cg_solve(basis, g_r, part, lam, torch.from_numpy(b[glob]).cuda(), x, rtol=rtol, maxit=20 * ng, precond=precond)
+        sol[r] = x.cpu().numpy()
+    _run_ranks(world, rank_body)
+    ref = G @ u
+    cond = np.linalg.cond(G)
+    for r in range(world):
+        glob = ranks[r][3]
+        assert np.abs(out[r] - ref[glob]).max() <= 1e-12 * np.abs(ref).max(), r
+        assert its[r] == its[0] and its[r][1] <= rtol                      # identical on every rank
+        assert np.abs(sol[r] - xs[glob]).max() <= 10 * cond * rtol * np.abs(xs).max(), (r, its[r], cond)
+        if dirichlet:
+            assert np.abs(sol[r][np.isin(glob, bd.numpy())]).max() == 0.0
+    # same Krylov iteration as the one-rank solve (sums in another order: the count may differ by a step or two)
+    assert abs(its[0][0] - it1) <= max(3, it1 // 20), (its[0], it1)
+    assert comm.calls > 3 * its[0][0]                                      # interface + two scalar all-reduces per iteration
+
+
+def test_partition_of_one_rank_equals_cg_solve(nk):
+    """world = 1: no shared dofs, the all-reduce is the identity: nk_part_cg_solve reproduces nk_cg_solve's iteration."""
+    el, A, J, basis, geom, l2g, ng = setup(nk, 2, 3, True)
+    gs = nk.GatherScatter(l2g, ng)
+    p = asm.partition_l2g(l2g, ng, 1)[0]
+    assert p["n_interface"] == 0 and torch.equal(p["l2g"], l2g)
+    calls = []
+    part = nk.Partition(gs, p["shared_dof"], p["shared_slot"], p["shared_mult"], 0, lambda t: calls.append(t.numel()))
+    b = torch.from_numpy(np.random.Generator(np.random.Philox(5)).standard_normal(ng)).cuda()
+    x0, x1 = torch.zeros_like(b), torch.zeros_like(b)
+    it0, rel0 = nk.cg_solve(basis, geom, gs, 1.0, b, x0, rtol=1e-10, maxit=5000, precond=1)
+    it1, rel1 = nk.part_cg_solve(basis, geom, part, 1.0, b, x1, rtol=1e-10, maxit=5000, precond=1)
+    assert abs(it1 - it0) <= 2 and rel1 <= 1e-10
+    assert float((x1 - x0).abs().max()) <= 1e-8 * float(x0.abs().max())
+    assert set(calls) <= {1, 2}                                            # only the scalar reductions were called
+    with pytest.raises(nk.NkError):                                        # a slot listed twice
+        nk.Partition(gs, torch.tensor([0, 1]), torch.tensor([0, 0]), torch.tensor([2, 2], dtype=torch.int32), 2, lambda t: None)

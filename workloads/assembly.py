@@ -33,3 +33,40 @@ def hex_boundary_dofs(n, P):
     on = (g == 0) | (g == N1 - 1)
     m = on[:, None, None] | on[None, :, None] | on[None, None, :]
     return torch.nonzero(m.reshape(-1)).reshape(-1).to(torch.int64).contiguous()
+
+
+def partition_l2g(l2g, nglobal, world):
+    """Splits a mesh with local-to-global map `l2g` [nelem][nm] into `world` contiguous element ranges (the shards of
+    workloads.configs.shard) and describes each rank's share of the global system (DATA ONLY: integer bookkeeping).
+
+    Returns one dict per rank:
+      range          (lo, hi) element range
+      glob           int64 [nr]: global dof of every rank-local dof, ascending (the rank's numbering)
+      l2g            int64 [hi-lo][nm]: the rank's map in its own numbering
+      shared_dof     int64 [ns]: rank-local dofs that other ranks hold too (the interface), ascending
+      shared_slot    int64 [ns]: their position in the interface vector, the same on every rank
+      shared_mult    int32 [ns]: number of ranks that hold each of them (>= 2)
+      n_interface    length of the interface vector (dofs held by more than one rank)
+    """
+    nelem = l2g.shape[0]
+    bounds = [nelem * r // world for r in range(world + 1)]
+    held = torch.zeros(nglobal, dtype=torch.int32)
+    globs = []
+    for r in range(world):
+        g = torch.unique(l2g[bounds[r]:bounds[r + 1]].reshape(-1))      # sorted
+        globs.append(g)
+        held[g] += 1
+    iface = torch.nonzero(held > 1).reshape(-1)                         # ascending global ids
+    slot_of = torch.full((nglobal,), -1, dtype=torch.int64)
+    slot_of[iface] = torch.arange(iface.numel(), dtype=torch.int64)
+    parts = []
+    for r in range(world):
+        g = globs[r]
+        loc_of = torch.full((nglobal,), -1, dtype=torch.int64)
+        loc_of[g] = torch.arange(g.numel(), dtype=torch.int64)
+        sh = torch.nonzero(held[g] > 1).reshape(-1)
+        parts.append(dict(range=(bounds[r], bounds[r + 1]), glob=g.contiguous(),
+                          l2g=loc_of[l2g[bounds[r]:bounds[r + 1]]].contiguous(),
+                          shared_dof=sh.to(torch.int64).contiguous(), shared_slot=slot_of[g[sh]].contiguous(),
+                          shared_mult=held[g[sh]].to(torch.int32).contiguous(), n_interface=int(iface.numel())))
+    return parts
