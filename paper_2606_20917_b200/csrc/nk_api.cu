@@ -1007,6 +1007,7 @@ extern "C" void nk_count_launches_(int n)
 extern "C" int nk_helmholtz_apply_allocates_(const nk_basis* b, const nk_geom* g)
 {
     if (!b || !g) return 1;
+    if (b->jit) return 1;      // a basis outside the prebuilt table: its kernels are compiled and loaded on first use
     nk_status st = NK_OK;
     if (!use_dense(b, g->deformed, nk::OP_HELM, &st)) return st == NK_OK ? 0 : 1;
     if (!nk::dense_supported(b->t.Nm)) return 1;

@@ -123,3 +123,56 @@ def test_hp_mixed_batch_in_one_call(nk):
     torch.cuda.synchronize()
     for (shape, P, Q, deformed, n), (b, g, x, y), ref in zip(spec, blocks, refs):
         assert K.normwise_err(y.cpu().numpy(), ref) <= TOL, (shape, P, Q, deformed)
+
+
+@pytest.mark.parametrize("shape,P,Q,deformed", [(o.HEX, 4, 7, True), (o.HEX, 3, 4, False), (o.PRISM, 3, 6, True)])
+def test_every_entry_point_serves_a_specialised_basis(nk, shape, P, Q, deformed):
+    """the other entries of include/nk.h on a run-time specialised basis: the multi-field call (one launch, bit-identical
+    to the single-field one), the host entry (chunked launches over group ranges), repeatability, and, on hexes, the
+    assembled apply and CG solve; the entry that must not allocate refuses such a basis."""
+    from workloads import assembly as asm
+    lam = 1.25
+    el = K.element(shape, P, Q)
+    full = K.mesh(shape, 3)[0].shape[0]
+    take = torch.arange(full - (0 if shape == o.HEX else 3))
+    A, J = K.geometry(shape, P, 3, deformed, take=take, xi=el.xi)
+    ne = J.shape[0]
+    basis = nk.Basis(shape, P, Q)
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), deformed)
+    xs = [wl.coefficients(300 + f, ne, el.Nm) for f in range(3)]
+    refs = [o.helmholtz(el, A.numpy(), J.numpy(), lam, x.numpy()) for x in xs]
+    dx = [x.cuda() for x in xs]
+    dy = [torch.full_like(x, float("nan")) for x in dx]
+    nk.helmholtz_apply_fields(basis, geom, lam, dx, dy)          # compiles the multi-field instantiation
+    n0 = nk.launch_count()
+    nk.helmholtz_apply_fields(basis, geom, lam, dx, dy)
+    assert nk.launch_count() == n0 + 1
+    torch.cuda.synchronize()
+    for f in range(3):
+        assert K.normwise_err(dy[f].cpu().numpy(), refs[f]) <= TOL
+        y1 = torch.empty_like(dx[f])
+        nk.helmholtz_apply(basis, geom, lam, dx[f], y1)
+        y2 = torch.empty_like(dx[f])
+        nk.helmholtz_apply(basis, geom, lam, dx[f], y2)
+        assert torch.equal(y1, dy[f]) and torch.equal(y1, y2)
+    xh = xs[0].pin_memory()
+    yh = torch.full_like(xh, float("nan")).pin_memory()
+    nk.helmholtz_apply_host(basis, geom, lam, xh, yh)
+    assert K.normwise_err(yh.numpy(), refs[0]) <= TOL
+    if shape == o.HEX:
+        l2g, ng = asm.hex_l2g(3, P)
+        G = o.assembled_matrix(el, A.numpy(), J.numpy(), lam, l2g.numpy(), ng)
+        gs = nk.GatherScatter(l2g, ng)
+        rng = np.random.Generator(np.random.Philox(9))
+        u, b = rng.standard_normal(ng), rng.standard_normal(ng)
+        out = torch.full((ng,), float("nan"), dtype=torch.float64, device="cuda")
+        nk.assembled_helmholtz_apply(basis, geom, gs, lam, torch.from_numpy(u).cuda(), out)
+        ref = G @ u
+        assert np.abs(out.cpu().numpy() - ref).max() <= 1e-12 * np.abs(ref).max()
+        x = torch.zeros(ng, dtype=torch.float64, device="cuda")
+        iters, rel = nk.cg_solve(basis, geom, gs, lam, torch.from_numpy(b).cuda(), x, rtol=1e-10, maxit=20 * ng, precond=1)
+        xsol = np.linalg.solve(G, b)
+        assert rel <= 1e-10 and np.abs(x.cpu().numpy() - xsol).max() <= 10 * np.linalg.cond(G) * 1e-10 * np.abs(xsol).max()
+        with pytest.raises(nk.NkError) as ei:
+            nk.assembled_helmholtz_apply_static(basis, geom, gs, lam, torch.from_numpy(u).cuda(), out)
+        assert ei.value.code == 2
