@@ -66,9 +66,9 @@ typedef struct nk_geom nk_geom;   /* opaque: nelem, deformed flag, repacked devi
 /* ---- basis / quadrature precompute (host only; needs no GPU) ----------------------------------
  * Modified C0 basis (A7, A8) with Gauss-Lobatto-Legendre points on hexes, GLL x Gauss-Radau-Jacobi(1,0)
  * x GRJ(2,0) on tets, GLL x GLL x GRJ(1,0) on prisms (A9).  Prebuilt kernels: Q == P+2 with
- * hex P in 1..10, tet and prism P in 1..8.  Any other (P, Q) with 1 <= P <= 10, P+1 <= Q <= 12 whose tables fit the
- * kernel-parameter space (every hex; tets / prisms up to P = 9) is accepted too and its kernels are specialised at
- * run time on first use ("run-time specialisation" below); anything else returns NK_ERR_UNSUPPORTED.   */
+ * hex P in 1..10, tet and prism P in 1..8.  Any other (P, Q) with 1 <= P <= 10, P+1 <= Q <= 12 is accepted too, on every
+ * shape, and its kernels are specialised at run time on first use ("run-time specialisation" below); anything else
+ * returns NK_ERR_UNSUPPORTED.                                                                              */
 nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** out);
 nk_status nk_basis_destroy(nk_basis* b);
 int nk_basis_num_modes(const nk_basis* b);  /* Nm; -1 if b is NULL */
@@ -280,9 +280,9 @@ nk_status nk_basis_get_reference_matrix(const nk_basis* b, int c, double* host_o
  * libcuda are dlopen'ed (no link-time dependency), and a failure surfaces as NK_ERR_UNSUPPORTED at apply time.
  *  - Reference-matrix kernels (one number, the modes per element): csrc/nk_dense.cuh for a mode count outside the
  *    prebuilt table (tets P1..P8, trilinear hexes); cached per (device, modes, operator).
- *  - Sum-factorised kernels: nk_basis_create accepts ANY (shape, P, Q) with 1 <= P <= 10 and P+1 <= Q <= 12 whose basis
- *    tables fit the 32 KB kernel-parameter space (every hex; tets and prisms up to P = 9): nk_kernel<shape, P, deformed,
- *    operator, Q> is instantiated per first use with the launch rules of the prebuilt table (they depend on Q); cached
+ *  - Sum-factorised kernels: nk_basis_create accepts ANY (shape, P, Q) with 1 <= P <= 10 and P+1 <= Q <= 12 (tets and
+ *    prisms of order 10 keep one copy of their psi^b tables instead of two so that they fit the 32 KB kernel-parameter
+ *    space): nk_kernel<shape, P, deformed, operator, Q> is instantiated per first use with the launch rules of the prebuilt table (they depend on Q); cached
  *    per (device, shape, P, Q, deformed, operator).  Every operator of this header works on such a basis.
  * nk_jit_compile_check: compile the reference-matrix Helmholtz kernel for `nmodes` without loading it (needs NO GPU):
  * NVRTC's wall time in ms and the cubin size.  nk_jit_compile_check_kernel: the same for one sum-factorised

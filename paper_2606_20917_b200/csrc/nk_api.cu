@@ -265,12 +265,16 @@ extern "C" nk_status nk_basis_create(nk_shape shape, int P, int Q, nk_basis** ou
         f.push_back(shape == NK_TET ? t.w[2][i] * s * s : t.w[2][i] * s);
     }
     for (int i = 0; i < Q; ++i) f.push_back(shape != NK_HEX ? t.w[2][i] / (1.0 - t.z[2][i]) : 0.0);
-    // SimplexTabs: b3f, b3a (psi^b at the direction-3 points), b2f, b2a (direction 2; tet only)
+    // SimplexTabs: b3f, b3a (psi^b at the direction-3 points), b2f, b2a (direction 2; tet only); where two copies do not
+    // fit the kernel-parameter space (k_sx_dup: tets / prisms at P = 10) the adjoint copies shrink to one unused entry
     if (shape != NK_HEX) {
         std::vector<double>& x = b->sx_flat;
         const size_t n = (size_t)t.npair * Q;
-        for (int c = 0; c < 2; ++c) x.insert(x.end(), t.tab3.begin(), t.tab3.end());
+        const bool dup = nk::k_sx_dup((int)shape, nm, Q);
+        x.insert(x.end(), t.tab3.begin(), t.tab3.end());
+        if (dup) x.insert(x.end(), t.tab3.begin(), t.tab3.end()); else x.push_back(0.0);
         for (int c = 0; c < 2; ++c) {
+            if (c == 1 && !dup) { x.push_back(0.0); break; }
             if (shape == NK_TET) x.insert(x.end(), t.tab2.begin(), t.tab2.end());
             else x.insert(x.end(), n, 0.0);
         }

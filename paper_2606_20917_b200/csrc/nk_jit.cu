@@ -7,7 +7,7 @@
 //     Nm outside the prebuilt table (prisms, hexes of order >= 2, ... when nk_set_affine_simplex_form(2) asks for the
 //     reference-matrix form there), cached per (device, Nm, operator);
 //   * the sum-factorised kernel template nk_kernel<shape, P, deformed, op, Q> (nk_kernel_body.cuh and its stage files) is
-//     compiled for a (shape, P, Q) outside the table -- any P+1 <= Q <= 12, tets and prisms of order 9 -- one
+//     compiled for a (shape, P, Q) outside the table -- any P+1 <= Q <= 12, tets and prisms of order 9 and 10 -- one
 //     instantiation per first use, cached per (device, shape, P, Q, deformed, operator); second half of this file.
 // Cubins are loaded through the driver API.
 // libnvrtc and libcuda are opened with dlopen: libnk.so has no link-time dependency on either, loads on a machine
@@ -312,7 +312,7 @@ bool dense_jit_launch(int nmodes, int kind, const DenseArgs& a, cudaStream_t str
 
 
 // =====================================================================================================================
-// Sum-factorised kernels (nk_kernel_body.cuh) for a (shape, P, Q) outside the prebuilt table: tets / prisms of order 9,
+// Sum-factorised kernels (nk_kernel_body.cuh) for a (shape, P, Q) outside the prebuilt table: tets / prisms of order 9 and 10,
 // any Q != P+2 (P+1 <= Q <= 12).  The kernel template takes Q as a parameter and its launch rules (Tune / TuneOp) are
 // functions of Q, so the host reads the configuration of any triple from the same templates (table below, no GPU needed)
 // and NVRTC instantiates exactly one nk_kernel<shape, P, deformed, op, Q> per first use.
@@ -338,6 +338,8 @@ void fill_info(JitInfo& o)
     fill_ops<SHAPE, P, Q, 1>(o, std::make_integer_sequence<int, OP_COUNT>{});
     o.tabs_bytes = sizeof(DenseTabs<P + 1, Q, SHAPE == K_HEX>);
     o.sx_bytes = sizeof(typename SimplexTabsFor<SHAPE, P + 1, Q>::type);
+    o.sx_dup = k_sx_dup(SHAPE, P + 1, Q);
+    static_assert(sizeof(DenseTabs<P + 1, Q, SHAPE == K_HEX>) == sizeof(double) * k_dense_doubles(P + 1, Q, SHAPE == K_HEX), "k_dense_doubles out of date");
 }
 // Q = P+1 .. kJitMaxQ
 template <int SHAPE, int P, int... DQ>

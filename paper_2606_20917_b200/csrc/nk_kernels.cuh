@@ -64,7 +64,7 @@ struct Tune {
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : 4)
+    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : Q <= 11 ? 4 : 2)   // simplices at Q = 12: shared memory
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
@@ -237,14 +237,26 @@ __host__ __device__ constexpr int k_prism_mode0(int nm, int p, int q)
 // psi^b tables of the collapsed directions (A7), constant-bank operands of the simplex stages.
 // Row = k_pair(a,b), Q entries per row (contiguous in the point index).  Forward and adjoint stages have
 // their own copies (same reason as DenseTabs).  NRQ = npair*Q on simplices, 1 on hexes (unused).
-template <int NRQ>
+// DUP = false: ONE copy serves both (the adjoint accessors return the forward arrays).  Only where two copies do not fit
+// the 32 KB kernel-parameter space next to DenseTabs: tets and prisms at P = 10, Q = 12 (run-time specialised only).
+template <int NRQ, bool DUPL = true>
 struct SimplexTabs {
-    double b3f[NRQ], b3a[NRQ]; // psi^b_{s,r}(eta3_k): tet s = p+q, prism s = p
-    double b2f[NRQ], b2a[NRQ]; // psi^b_{p,q}(eta2_j): tet only
+    static constexpr bool DUP = DUPL;
+    double b3f[NRQ], b3a[DUPL ? NRQ : 1]; // psi^b_{s,r}(eta3_k): tet s = p+q, prism s = p
+    double b2f[NRQ], b2a[DUPL ? NRQ : 1]; // psi^b_{p,q}(eta2_j): tet only
+    __device__ __forceinline__ const double* a3() const { if constexpr (DUPL) return b3a; else return b3f; }
+    __device__ __forceinline__ const double* a2() const { if constexpr (DUPL) return b2a; else return b2f; }
 };
+// doubles of DenseTabs<NM, Q, HEXK> (declaration order: Ba, BaT, KM, D, DT, w, aux)
+__host__ __device__ constexpr int k_dense_doubles(int nm, int Q, bool hexk) { return 6 * Q * nm + 12 * (hexk ? nm * nm : 1) + 6 * Q * Q + 10 * Q; }
+// do two copies of the psi^b tables fit the kernel-parameter space (32000 B with 512 B left for KArgs)?
+__host__ __device__ constexpr bool k_sx_dup(int shape, int nm, int Q)
+{
+    return shape == K_HEX || (k_dense_doubles(nm, Q, false) + 4 * (nm * (nm + 1) / 2) * Q) * 8 + 512 <= 32000;
+}
 template <int SHAPE, int NM, int Q>
 struct SimplexTabsFor {
-    using type = SimplexTabs<(SHAPE == K_HEX) ? 1 : (NM * (NM + 1) / 2) * Q>;
+    using type = SimplexTabs<(SHAPE == K_HEX) ? 1 : (NM * (NM + 1) / 2) * Q, k_sx_dup(SHAPE, NM, Q)>;
 };
 
 enum { K_MAX_FIELDS = 8 };

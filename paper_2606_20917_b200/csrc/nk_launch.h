@@ -27,6 +27,7 @@ struct JitInfo {
     int E[2];                       // interleave width of the geometry stream [deformed] (Tune<...>::E)
     JitOpCfg op[2][OP_COUNT];       // [deformed][op]
     size_t tabs_bytes, sx_bytes;    // sizeof(DenseTabs), sizeof(SimplexTabs) of this (shape, P, Q)
+    bool sx_dup;                    // SimplexTabs holds separate adjoint copies (k_sx_dup)
 };
 enum { kJitMaxP = 10, kJitMaxQ = 12 };
 } // namespace nk

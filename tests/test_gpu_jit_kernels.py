@@ -73,11 +73,13 @@ def test_run_time_kernels_are_counted(nk):
 
 
 @pytest.mark.parametrize("shape", [o.TET, o.PRISM])
-def test_tet_and_prism_order_9(nk, shape):
+def test_tet_and_prism_orders_9_and_10(nk, shape):
     """orders beyond the prebuilt simplex table (P <= 8; SURVEY section 5 asked for 1..10): P = 9 with
-    Q = 11, affine (sum-factorised form) and deformed."""
+    Q = 11 and P = 10 with Q = 12 (one copy of the psi^b tables there: two do not fit the kernel-parameter space), affine
+    (sum-factorised form) and deformed."""
     for deformed in (False, True):
         run_case(nk, shape, 9, 11, 2, deformed, ("helmholtz", "bwdtrans", "iprod", "physderiv", "iprod_deriv"), lam=10.0, zhi=1)
+        run_case(nk, shape, 10, 12, 2, deformed, ("helmholtz", "bwdtrans", "iprod_deriv"), lam=10.0, zhi=1)
 
 
 def test_specialised_equals_prebuilt_template(nk):
@@ -96,7 +98,7 @@ def test_specialised_equals_prebuilt_template(nk):
 
 
 def test_unsupported_triples_are_refused(nk):
-    for shape, P, Q in ((o.HEX, 3, 3), (o.HEX, 11, 13), (o.TET, 10, 12), (o.HEX, 4, 13)):
+    for shape, P, Q in ((o.HEX, 3, 3), (o.HEX, 11, 13), (o.TET, 10, 13), (o.HEX, 4, 13), (o.PRISM, 11, 12)):
         with pytest.raises(nk.NkError) as ei:
             nk.Basis(shape, P, Q)
         assert ei.value.code == 2      # NK_ERR_UNSUPPORTED

@@ -25,7 +25,7 @@ def test_exports_every_declared_symbol():
     assert declared == set(nk.DECLARED_SYMBOLS), declared ^ set(nk.DECLARED_SYMBOLS)
 
 
-@pytest.mark.parametrize("shape,P,Q", [(o.HEX, 4, 5), (o.HEX, 2, 6), (o.TET, 3, 6), (o.TET, 9, 11), (o.PRISM, 4, 7), (o.PRISM, 9, 11)])
+@pytest.mark.parametrize("shape,P,Q", [(o.HEX, 4, 5), (o.HEX, 2, 6), (o.TET, 3, 6), (o.TET, 9, 11), (o.PRISM, 4, 7), (o.PRISM, 9, 11), (o.TET, 10, 12), (o.PRISM, 10, 12)])
 def test_host_tables_of_run_time_specialised_bases(shape, P, Q):
     """(shape, P, Q) outside the prebuilt Q = P+2 table (kernels specialised at run time, csrc/nk_jit.cu): the host
     precompute is the same code and is checked against the oracle's tables the same way; the interleave widths come
@@ -90,7 +90,7 @@ def test_error_codes_and_no_cpu_fallback():
     with pytest.raises(nk.NkError) as ei:
         nk.Basis(o.HEX, 11)
     assert ei.value.code == 2
-    for shape, P, Q in ((o.TET, 4, 4), (o.HEX, 4, 13), (o.TET, 10, 12)):   # Q < P+1; Q > 12; tables beyond the parameter space
+    for shape, P, Q in ((o.TET, 4, 4), (o.HEX, 4, 13), (o.PRISM, 11, 12)):   # Q < P+1; Q > 12; P > 10
         with pytest.raises(nk.NkError) as ei:
             nk.Basis(shape, P, Q=Q)
         assert ei.value.code == 2
