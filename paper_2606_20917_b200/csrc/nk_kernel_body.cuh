@@ -88,6 +88,11 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
     double* __restrict__ Z = S0 + (size_t)(T::KRON ? 1 : 2) * NQP * E;
     double* __restrict__ RG = S0 + (size_t)3 * NQP * E;      // geometry ring [RING][7][threads] (T::RING > 0 only)
     (void)RG;
+    // psi^b tables of the triangular stages in shared memory (T::SXS): b3 then b2, behind the arrays and the ring
+    constexpr bool SXS = T::SXS && !KRON;
+    constexpr int NRQ = (NM * (NM + 1) / 2) * Q;
+    double* __restrict__ SXT = S0 + (size_t)3 * NQP * E + (T::RING > 0 ? (size_t)T::NT * T::RING * 7 : 0);
+    (void)SXT; (void)NRQ;
     const int e = tid % E, slot = tid / E;
     constexpr bool active = true;
 #define NK_SYNC() __syncthreads()
@@ -137,6 +142,13 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
                     const unsigned bytes = (unsigned)(cnt * NIN * sizeof(double)) & ~15u;
                     if (bytes && (reinterpret_cast<size_t>(base + e0 * NIN) & 15) == 0) l2_prefetch(base + e0 * NIN, bytes);
                 }
+            }
+        }
+        if constexpr (SXS) {
+            // every block copies the two tables once (a block barrier follows before the first triangular stage)
+            for (int i = tid; i < NRQ; i += T::NT) {
+                SXT[i] = st.b3f[i];
+                if constexpr (SHAPE == K_TET) SXT[NRQ + i] = st.b2f[i];
             }
         }
         // ================= input side =================

@@ -121,7 +121,21 @@ struct Tune {
     // simplices from Q = 9 (config 5 P7 / P8 +3 / +9 %); below, the two forms are within 1-3 % and the row form stays
     static constexpr bool COLS = SHAPE == K_HEX ? (Q >= 10 && (DEF || Q != 11)) : Q >= 9;
 #endif
-    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double);
+    // SXS: the psi^b tables of the triangular stages (nk_stage_sx.inc) read from a shared-memory copy that every block makes
+    // at entry ([2][npair * Q] doubles behind the point arrays and the ring) instead of as constant-bank operands.  In those
+    // stages every warp works on its own class with its own table rows, once per block: the constant loads (LDCU) find nothing
+    // in the constant cache that another warp has just used, and an ablation on B200 showed the four triangular stages of the
+    // deformed tet P5 kernel cost 35 % of its time for 8 % of its DFMA (profiles/r2_notes.md section 14).  From shared
+    // memory the same operands cost a fixed LDS latency.  B200 sweep (fraction of HBM, constant bank -> shared): tets P5 0.62 ->
+    // 0.69, P6 0.64 -> 0.66, P7 0.36 -> 0.38, P8 0.36 -> 0.37; prisms P6 0.70 -> 0.71, P7 0.57 -> 0.63; it LOSES 2-9 % at P1..P4
+    // (short blocks: the copy costs more than the few operands save) and on prisms at P5 and P8.
+#if defined(NK_TUNE_SXS)
+    static constexpr bool SXS = SHAPE != K_HEX && NK_TUNE_SXS != 0;
+#else
+    static constexpr bool SXS = DEF && ((SHAPE == K_TET && Q >= 7 && Q <= 10) || (SHAPE == K_PRISM && (Q == 8 || Q == 9)));
+#endif
+    static constexpr size_t smem_sx = SXS ? (size_t)2 * (NM * (NM + 1) / 2) * Q * sizeof(double) : 0;
+    static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double) + smem_sx;
 #if defined(NK_TUNE_MINB)
     static constexpr int MINB = NK_TUNE_MINB;
 #else
