@@ -93,6 +93,8 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
     constexpr int NRQ = (NM * (NM + 1) / 2) * Q;
     double* __restrict__ SXT = S0 + (size_t)3 * NQP * E + (T::RING > 0 ? (size_t)T::NT * T::RING * 7 : 0);
     (void)SXT; (void)NRQ;
+    // nk_stage_s3.inc does the q-sum of S2 itself (not for the mass operator, whose S3 writes W2 over T2 in place)
+    constexpr bool FUSE23 = SXS && T::FUSE23 && IN_COEFF && OP != OP_MASS;
     const int e = tid % E, slot = tid / E;
     constexpr bool active = true;
 #define NK_SYNC() __syncthreads()
@@ -202,7 +204,9 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
             }
             NK_SYNC();
             // a2/S2: sum over q:  T1 -> T2[p][j][k] in X
-            if constexpr (!SP2) {
+            if constexpr (FUSE23) {
+                // fused into S3 below: T1 was written to X by S1
+            } else if constexpr (!SP2) {
                 NK_FOR(l, NM * Q) {
                     const int p = l / Q, k = l - p * Q;
                     double c[NM];
@@ -217,7 +221,7 @@ nk_kernel(const __grid_constant__ DenseTabs<P + 1, QQ, SHAPE == K_HEX> tabs,
 #include "nk_stage_sx.inc"
 #undef NK_SX_STAGE
             }
-            NK_SYNC();
+            if constexpr (!FUSE23) NK_SYNC();
 #include "nk_stage_s3.inc"
             } // !KRON
         } else {

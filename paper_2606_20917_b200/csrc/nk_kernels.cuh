@@ -134,6 +134,14 @@ struct Tune {
 #else
     static constexpr bool SXS = DEF && ((SHAPE == K_TET && Q >= 7 && Q <= 10) || (SHAPE == K_PRISM && (Q == 8 || Q == 9)));
 #endif
+    // FUSE23 (tets with SXS): the q-sum S2 is done by the S3 thread for its own (j,k) line -- 21 more FMA per thread with
+    // psi^b_{pq}(eta2_j) read per lane from the shared-memory table -- instead of in a triangular stage of its own: one stage
+    // and one block barrier less, every thread busy (the S2 stage keeps one warp per p with 6..1 q-terms)
+#if defined(NK_TUNE_FUSE23)
+    static constexpr bool FUSE23 = SXS && SHAPE == K_TET && NK_TUNE_FUSE23 != 0;
+#else
+    static constexpr bool FUSE23 = SXS && SHAPE == K_TET;
+#endif
     static constexpr size_t smem_sx = SXS ? (size_t)2 * (NM * (NM + 1) / 2) * Q * sizeof(double) : 0;
     static constexpr size_t smem_grid = (size_t)3 * NQP * E * sizeof(double) + smem_sx;
 #if defined(NK_TUNE_MINB)
