@@ -64,7 +64,9 @@ struct Tune {
 #if defined(NK_TUNE_E)
     static constexpr int E = NK_TUNE_E;
 #else
-    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? 8 : Q <= 11 ? 4 : 2)   // simplices at Q = 12: shared memory
+    // (deformed prisms at Q = 8: 4 since their psi^b tables sit in shared memory -- 256 threads, three blocks per SM: 0.71 -> 0.76 of HBM;
+    //  tets keep 8 there: 0.67 against 0.66)
+    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? (SHAPE == K_PRISM ? 4 : 8) : Q <= 11 ? 4 : 2)   // simplices at Q = 12: shared memory
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
