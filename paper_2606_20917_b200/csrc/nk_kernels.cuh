@@ -153,11 +153,12 @@ struct Tune {
     // deformed workload (profiles/r2_notes.md section 7): hexes 96 except Q = 4 (64: cfg2:2 +4 %), Q = 7 and Q = 10
     // (80: cfg2:5 +5 %, cfg2:8 +7 %); simplices 72 except Q = 6 and Q = 8 (64: cfg5:4 +6 %, cfg5:6 +12 %, where 64
     // registers let a second 512-thread block fit); tets at Q = 7: 56 since their psi^b tables sit in shared memory (SXS below:
-    // five blocks of 224 threads per SM instead of four, 16 B of spills; config 5's tet launch 0.721 -> 0.741 of HBM)
+    // five blocks of 224 threads per SM instead of four, 16 B of spills; config 5's tet launch 0.721 -> 0.741 of HBM), and at
+    // Q = 9: 64 (a second 512-thread block per SM: tet P7 launch 0.38 -> 0.49)
 #if defined(NK_TUNE_REGS)
     static constexpr int REGS = NK_TUNE_REGS;
 #else
-    static constexpr int REGS = DEF ? (SHAPE == K_HEX ? (Q == 4 ? 64 : (Q == 7 || Q == 10) ? 80 : 96) : (Q == 6 || Q == 8) ? 64 : (SHAPE == K_TET && Q == 7) ? 56 : 72)
+    static constexpr int REGS = DEF ? (SHAPE == K_HEX ? (Q == 4 ? 64 : (Q == 7 || Q == 10) ? 80 : 96) : (Q == 6 || Q == 8 || (SHAPE == K_TET && Q == 9)) ? 64 : (SHAPE == K_TET && Q == 7) ? 56 : 72)
                                     : Q <= 6 ? 56 : 64;
 #endif
     static constexpr int MINB_smem = (int)((227 * 1024) / (smem_grid + smem_ring + 1024));
