@@ -65,8 +65,9 @@ struct Tune {
     static constexpr int E = NK_TUNE_E;
 #else
     // (deformed prisms at Q = 8: 4 since their psi^b tables sit in shared memory -- 256 threads, three blocks per SM: 0.71 -> 0.76 of HBM;
-    //  tets keep 8 there: 0.67 against 0.66)
-    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? (SHAPE == K_PRISM ? 4 : 8) : Q <= 11 ? 4 : 2)   // simplices at Q = 12: shared memory
+    //  tets keep 8 there: 0.67 against 0.66; simplices at Q = 10: 8 without the geometry ring -- one block of 864 threads per SM --
+    //  against 4 with it: tet P8 launch 0.37 -> 0.49, prism P8 0.46 -> 0.55)
+    static constexpr int E = DEF ? (Q <= 4 ? 8 : Q <= 7 ? 4 : SHAPE == K_HEX ? 2 : Q <= 8 ? (SHAPE == K_PRISM ? 4 : 8) : Q == 10 ? 8 : Q <= 11 ? 4 : 2)   // simplices at Q = 12: shared memory
                                  : (Q <= 3 ? 32 : Q <= 4 ? (SHAPE == K_HEX ? 16 : 8) : Q <= 5 ? 8 : Q <= 7 ? 4 : Q <= 8 ? 8
                                     : Q <= 10 ? 4 : 2);
 #endif
@@ -102,8 +103,10 @@ struct Tune {
 #else
     // B200 sweep (profiles/r2_notes.md): the ring costs 7 LDGSTS + 7 LDS per point instead of 7 LDG and loses wherever the
     // L2 prefetch alone keeps pass C fed (hexes at every order: cfg2 49.0 -> 42.8; simplices up to Q = 9: cfg5 19.5 -> 16.3);
-    // it wins on the simplices at Q = 10 (cfg5:8 10.2 -> 11.6 GDoF/s), where few warps are resident to hide the L2 latency
-    static constexpr int RING = (DEF && SHAPE != K_HEX && Q >= 10) ? 2 : 0;
+    // it won on the simplices at Q = 10 with four elements per block (cfg5:8 10.2 -> 11.6 GDoF/s), where few warps were resident
+    // to hide the L2 latency; eight elements per block without it do better still (12.6 -> 15.8, see E above), so the ring is
+    // left to Q >= 11 (run-time specialised orders 9 and 10), where eight elements do not fit the shared memory
+    static constexpr int RING = (DEF && SHAPE != K_HEX && Q >= 11) ? 2 : 0;
 #endif
     static constexpr size_t smem_ring = (size_t)NT * RING * 7 * sizeof(double);
     // EARLY: number of k-planes of the thread's pass-C line whose 7 metric entries are requested BEFORE the barrier in
