@@ -115,7 +115,8 @@ struct Tune {
 #if defined(NK_TUNE_EARLY)
     static constexpr int EARLY = (DEF && RING == 0) ? (NK_TUNE_EARLY < Q ? NK_TUNE_EARLY : Q) : 0;
 #else
-    static constexpr int EARLY = (DEF && RING == 0) ? (SHAPE != K_HEX ? 1 : Q == 9 ? 2 : 0) : 0;
+    // (simplices at Q = 8, re-swept with the shared-memory tables: two planes -- prism P6 launch 0.76 -> 0.83 of HBM, tet P6 0.67 -> 0.70)
+    static constexpr int EARLY = (DEF && RING == 0) ? (SHAPE != K_HEX ? (Q == 8 ? 2 : 1) : Q == 9 ? 2 : 0) : 0;
 #endif
     // COLS: form of the 1-D contractions (contract below): input-outermost over the transposed tables
 #if defined(NK_TUNE_COLS)
