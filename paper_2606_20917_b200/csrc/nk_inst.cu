@@ -58,10 +58,13 @@ static cudaError_t launch(const double* tabs_flat, const double* sx_flat, const 
     // L2 prefetch distance = 1/8 of the co-resident blocks (B200 sweep, profiles/r1_notes.md: flat between 3 %
     // and 25 %; at 100 % a third of the prefetched lines are evicted before use and re-read from DRAM).
     // NK_PREFETCH_PCT rescales it (percent of the co-resident blocks; 0 = off).
-    static const int pf_pct = [] {
+    // Kernels with ONE block per SM (deformed simplices at Q = 10: 864 threads, 218 KB) want the group only two or three blocks
+    // ahead (2 %): hybrid P8 mesh 0.519 -> 0.552 of HBM; with several blocks per SM 3..12 % are within 1 % of each other.
+    static const int pf_env = [] {
         const char* ev = std::getenv("NK_PREFETCH_PCT");
-        return ev ? std::atoi(ev) : 12;
+        return ev ? std::atoi(ev) : -1;
     }();
+    const int pf_pct = pf_env >= 0 ? pf_env : (blocks_per_sm == 1 ? 2 : 12);
     b.pf_dist = pf_pct > 0 ? (int)((long long)num_sms * blocks_per_sm * pf_pct / 100) + 1 : 0x3fffffff;
     const long long units = (long long)a.grid_groups * (a.nfields > 1 ? a.nfields : 1);   // (group, field) pairs
     const long long nblocks = units;

@@ -466,7 +466,7 @@ bool sumfac_jit_launch(const JitInfo& info, int def, int op, const double* tabs_
     if (a.grid_groups <= 0) return true;
     KArgs b = a;
     // L2 prefetch distance: the rule of the prebuilt kernels (nk_inst.cu)
-    b.pf_dist = (int)((long long)num_sms * L.blocks_per_sm * 12 / 100) + 1;
+    b.pf_dist = (int)((long long)num_sms * L.blocks_per_sm * (L.blocks_per_sm == 1 ? 2 : 12) / 100) + 1;
     const long long units = (long long)a.grid_groups * (a.nfields > 1 ? a.nfields : 1);
     if (units > 0x7fffffffLL) {
         *err = "too many groups";
