@@ -299,6 +299,34 @@ def test_helmholtz_host_entry(nk, deformed):
     assert K.normwise_err(y.numpy(), ref) <= TOL
 
 
+@pytest.mark.parametrize("shape,P", [(o.TET, 5), (o.TET, 6), (o.PRISM, 6), (o.TET, 8), (o.PRISM, 8)])
+def test_high_order_deformed_simplices_fields_and_repeatability(nk, shape, P):
+    """the deformed simplex kernels whose psi^b tables sit in shared memory (tets from P5, with S2 folded into S3; prisms at
+    P6, P7) and the wide blocks at P8: single-field and multi-field calls against the oracle, bit-identical to each other
+    and over repeated launches (a race on the shared table copy or on T1 in X would show as run-to-run noise)."""
+    lam, nf = 1.5, 2
+    el = K.element(shape, P)
+    A, J = K.geometry(shape, P, 2, True, zhi=1)
+    ne = J.shape[0]
+    basis = nk.Basis(shape, P)
+    geom = nk.Geom(basis, A.cuda(), J.cuda(), True)
+    xs = [wl.coefficients(400 + f, ne, el.Nm) for f in range(nf)]
+    dx = [x.cuda() for x in xs]
+    dy = [torch.full_like(x, float("nan")) for x in dx]
+    nk.helmholtz_apply_fields(basis, geom, lam, dx, dy)
+    torch.cuda.synchronize()
+    for f in range(nf):
+        ref = o.helmholtz(el, A.numpy(), J.numpy(), lam, xs[f].numpy())
+        assert K.normwise_err(dy[f].cpu().numpy(), ref) <= TOL
+        for _ in range(5):
+            y1 = torch.full_like(dx[f], float("nan"))
+            nk.helmholtz_apply(basis, geom, lam, dx[f], y1)
+            assert torch.equal(y1, dy[f])
+    for op in ("mass", "laplacian", "bwdtrans"):          # the operators that share the forward stages
+        x = K.make_input(op, 500, ne, el)
+        assert K.op_err(op, K.gpu_op(nk, op, basis, geom, lam, x), K.oracle_op(op, el, A, J, lam, x)) <= TOL, op
+
+
 @pytest.mark.parametrize("shape,deformed", [(o.HEX, True), (o.HEX, False), (o.TET, False), (o.PRISM, True)])
 def test_helmholtz_fields(nk, shape, deformed):
     """nk_helmholtz_apply_fields (multi-field block): each field equals the oracle's Helmholtz of that
